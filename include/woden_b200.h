@@ -1,0 +1,167 @@
+/* woden_b200.h -- C ABI of libwoden_b200.so: direct measurement-equation visibility
+ * prediction (the WODEN hot path of Line et al. 2020, arXiv:2005.09316) on one B200.
+ *
+ * Citations are PAPER.md line numbers (text of the paper) and DESIGN.md readings (G1-G14).
+ *
+ * What every predict call computes, for each baseline b, time step t and channel f
+ * (Eq 9 / Eq 11, primary beam B == 1, :125):
+ *
+ *   V(b,t,f) = sum_j  S_j(nu_f) * xi_j(u,v) * exp(-2 pi i (u l_j + v m_j + w (n_j - 1)))
+ *
+ *   (u,v,w)  = (u_m,v_m,w_m)[t][b] * nu_f / c      wavelengths; "u,v,w only differ in
+ *                                                  frequency by a scaling factor" (:161)
+ *   n_j      = sqrt(1 - l_j^2 - m_j^2)             (:115)
+ *   S_j(nu)  = s0_j * (nu / ref_freq)^alpha_j      single spectral index per source (:169, :365)
+ *   xi_j     = 1                                                         point source
+ *            = exp(-pi^2/(4 ln 2) (kx^2 maj^2 + ky^2 min^2)),
+ *              kx = cos(pa) v + sin(pa) u,  ky = -sin(pa) v + cos(pa) u   Gaussian, Eq 12-14 (:141-146)
+ *            = sum_q coeff_q i^(n1_q+n2_q) h_{n1_q}(beta1 K kx') h_{n2_q}(beta2 K ky'),
+ *              K = pi / sqrt(2 ln 2), kx', ky' as above from (u',v')     shapelet, Eq 15-17 (:150-157)
+ *              h_p(x) = H_p(x) exp(-x^2/2) / sqrt(2^p p!)                 Eq 1/3 (:51, :60), reading G2
+ *              (u',v') = M_j (u,v,w)^T, or (u,v) when uv_basis == NULL    (:157), reading G4
+ *
+ * Conventions (G6, G7): l, m direction cosines; angles in radians; maj/min are FWHM;
+ * pa is measured from North through East; c = 299792458 m/s; flux in Jy.  A shapelet with the
+ * single coefficient (0,0) = 1 and beta1 = maj, beta2 = min IS the Gaussian (:159).
+ *
+ * Memory: pointers marked DEVICE must be device memory on the context's GPU (e.g. a torch
+ * tensor's data_ptr()); pointers marked HOST are ordinary host memory read before the call
+ * returns.  The library never frees or keeps caller pointers after the call's work has run.
+ * Device calls only enqueue work on `cuda_stream` (a cudaStream_t, NULL = legacy default
+ * stream) and return without synchronising; internal scratch belongs to the context, so one
+ * context serves one stream at a time.
+ *
+ * Output layout: complex64 interleaved (re, im), vis[((t * n_freqs) + f) * n_baselines + b].
+ *
+ * There is no CPU fallback anywhere: without a CUDA device every entry point that needs one
+ * returns WODEN_ERR_CUDA.
+ */
+#ifndef WODEN_B200_H
+#define WODEN_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WODEN_OK                 0
+#define WODEN_ERR_NULL          -1   /* a required pointer is NULL                              */
+#define WODEN_ERR_DIM           -2   /* a size is non-positive / inconsistent / too large       */
+#define WODEN_ERR_ORDER         -3   /* p_max outside 0..WODEN_MAX_ORDER                        */
+#define WODEN_ERR_CUDA          -4   /* CUDA allocation / launch / copy failed (woden_last_error) */
+#define WODEN_ERR_UNIMPLEMENTED -5
+#define WODEN_ERR_DATA          -6   /* woden_check(): a device-side precondition was violated  */
+
+#define WODEN_MAX_ORDER 100          /* largest shapelet order n1 + n2 (paper uses <= 86, :183) */
+
+typedef struct woden_ctx woden_ctx;  /* owns internal device scratch only */
+
+/* Create / destroy a context bound to CUDA device `cuda_device`. */
+int woden_create(woden_ctx **ctx, int cuda_device);
+int woden_destroy(woden_ctx *ctx);
+
+/* Static description of a status code; woden_last_error() adds the CUDA error string of the
+ * last WODEN_ERR_CUDA on this context ("" if none).  Both return pointers owned by the library. */
+const char *woden_strerror(int status);
+const char *woden_last_error(const woden_ctx *ctx);
+
+/* Synchronises the context's last stream and reports device-side precondition violations
+ * counted since the last check (l^2+m^2 >= 1, non-finite parameters, beta <= 0, shapelet
+ * orders above p_max): WODEN_OK or WODEN_ERR_DATA.  Not on the hot path. */
+int woden_check(woden_ctx *ctx);
+
+/* Algorithm selection (measurement / testing).  Default WODEN_PATH_AUTO.
+ *   AUTO    : channel-walking fast path when freqs_hz is uniformly spaced, else general
+ *   GENERAL : always one sin/cos (and one exp2 for Gaussians) per component x visibility
+ * Both meet the same parity tolerance. */
+#define WODEN_PATH_AUTO    0
+#define WODEN_PATH_GENERAL 1
+int woden_set_path(woden_ctx *ctx, int path);
+
+/* Baseline coordinates and channels ("array layout and observation parameters"). */
+typedef struct {
+    int n_baselines, n_times, n_freqs;
+    const double *u_m, *v_m, *w_m;  /* DEVICE [n_times][n_baselines], metres, phase-centre frame */
+    const double *freqs_hz;         /* HOST   [n_freqs], any spacing, each > 0                    */
+} woden_uvw;
+
+/* Eq 9.  n components; l, m, s0_jy, alpha: DEVICE [n].
+ * vis: DEVICE complex64 [n_times][n_freqs][n_baselines].  accumulate = 0 overwrites vis,
+ * 1 adds into it.  n == 0: zero-fill (accumulate = 0) or no-op (accumulate = 1). */
+int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n,
+                         const double *l, const double *m,
+                         const double *s0_jy, const double *alpha, double ref_freq_hz,
+                         float *vis, int accumulate, void *cuda_stream);
+
+/* Eq 11 with the Gaussian envelope of Eq 12-14.
+ * maj_fwhm_rad, min_fwhm_rad (>= 0; both 0 is a point source, reading G13), pa_rad: DEVICE [n]. */
+int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n,
+                            const double *l, const double *m,
+                            const double *s0_jy, const double *alpha, double ref_freq_hz,
+                            const double *maj_fwhm_rad, const double *min_fwhm_rad,
+                            const double *pa_rad,
+                            float *vis, int accumulate, void *cuda_stream);
+
+/* Eq 11 with the shapelet envelope of Eq 15-17.
+ * beta1_rad, beta2_rad (> 0), pa_rad: DEVICE [n].
+ * uv_basis: DEVICE [n][6] row-major 2x3 M_j, or NULL for (u',v') = (u,v) (reading G4).
+ * coeff_offset: DEVICE int [n+1], CSR offsets into n1/n2/coeff, non-decreasing from 0;
+ * n_coeff = coeff_offset[n] is passed explicitly so the call never reads device memory.
+ * n1, n2: DEVICE int [n_coeff], n1, n2 >= 0 and n1 + n2 <= p_max (the paper's p_max, Eq 6 /
+ * Eq 15; reading G5); coeff: DEVICE [n_coeff], already divided by the
+ * component's integrated flux (:157).  Repeated (n1,n2) pairs add; missing pairs are zero
+ * (truncated models).  0 <= p_max <= WODEN_MAX_ORDER. */
+int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n,
+                            const double *l, const double *m,
+                            const double *s0_jy, const double *alpha, double ref_freq_hz,
+                            const double *beta1_rad, const double *beta2_rad, const double *pa_rad,
+                            const double *uv_basis,
+                            const int *coeff_offset, int n_coeff, int p_max,
+                            const int *n1, const int *n2, const double *coeff,
+                            float *vis, int accumulate, void *cuda_stream);
+
+/* Whole-sky convenience call on HOST buffers (the call a user with a sky model in host memory
+ * makes; bench.py's end-to-end number).  Every pointer inside the structs and `vis_host` is
+ * HOST memory (pinned or pageable).  Copies inputs to the GPU, runs the three predictors above
+ * (overwrite, then accumulate), copies vis back and synchronises `cuda_stream` before returning.
+ * A type with n == 0 may have NULL arrays. */
+typedef struct {
+    int n;
+    const double *l, *m, *s0_jy, *alpha;
+} woden_points_host;
+typedef struct {
+    int n;
+    const double *l, *m, *s0_jy, *alpha, *maj_fwhm_rad, *min_fwhm_rad, *pa_rad;
+} woden_gaussians_host;
+typedef struct {
+    int n, n_coeff, p_max;
+    const double *l, *m, *s0_jy, *alpha, *beta1_rad, *beta2_rad, *pa_rad;
+    const double *uv_basis;        /* [n][6] or NULL */
+    const int *coeff_offset, *n1, *n2;
+    const double *coeff;
+} woden_shapelets_host;
+
+int woden_simulate_host(woden_ctx *ctx,
+                        int n_baselines, int n_times, int n_freqs,
+                        const double *u_m, const double *v_m, const double *w_m, /* HOST [T][B] */
+                        const double *freqs_hz, double ref_freq_hz,
+                        const woden_points_host *points,        /* may be NULL */
+                        const woden_gaussians_host *gaussians,  /* may be NULL */
+                        const woden_shapelets_host *shapelets,  /* may be NULL */
+                        float *vis_host, void *cuda_stream);
+
+/* Pipe microbenchmarks used to MEASURE the roofline denominators.
+ * Runs `which` (WODEN_PIPE_*) for `iters` dependent-chain-free iterations on every SM and
+ * returns warp-instructions per second per GPU in *ops_per_s (thread-ops/s = x32) and the
+ * SM clock in Hz observed by clock64 over the run in *sm_clock_hz.  Synchronous. */
+#define WODEN_PIPE_FFMA   0
+#define WODEN_PIPE_MUFU   1   /* sin.approx + cos.approx + ex2.approx mix on the XU pipe */
+#define WODEN_PIPE_DFMA   2
+#define WODEN_PIPE_I2F    3
+#define WODEN_PIPE_LOP3   4
+int woden_pipe_rate(woden_ctx *ctx, int which, int iters, double *thread_ops_per_s,
+                    double *sm_clock_hz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WODEN_B200_H */

@@ -1,0 +1,297 @@
+"""ctypes binding of libwoden_b200.so (include/woden_b200.h).  Argument marshalling only: every
+step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory
+and streams (tensor.data_ptr(), torch.cuda.current_stream()).
+
+There is NO CPU fallback: if the shared library is missing this module raises on first use,
+and on a machine without a CUDA device `Woden()` raises `WodenError(WODEN_ERR_CUDA)`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwoden_b200.so")
+
+WODEN_OK = 0
+WODEN_ERR_NULL = -1
+WODEN_ERR_DIM = -2
+WODEN_ERR_ORDER = -3
+WODEN_ERR_CUDA = -4
+WODEN_ERR_UNIMPLEMENTED = -5
+WODEN_ERR_DATA = -6
+WODEN_MAX_ORDER = 100
+WODEN_PATH_AUTO = 0
+WODEN_PATH_GENERAL = 1
+PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA_IMM": 6, "F2F": 7,
+         "MUFU_EX2": 8, "MUFU_FFMA": 9}
+
+EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
+           "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
+           "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate"]
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+_vp = C.c_void_p
+
+
+class woden_uvw(C.Structure):
+    _fields_ = [("n_baselines", C.c_int), ("n_times", C.c_int), ("n_freqs", C.c_int),
+                ("u_m", _vp), ("v_m", _vp), ("w_m", _vp), ("freqs_hz", _dp)]
+
+
+class woden_points_host(C.Structure):
+    _fields_ = [("n", C.c_int), ("l", _dp), ("m", _dp), ("s0_jy", _dp), ("alpha", _dp)]
+
+
+class woden_gaussians_host(C.Structure):
+    _fields_ = [("n", C.c_int), ("l", _dp), ("m", _dp), ("s0_jy", _dp), ("alpha", _dp),
+                ("maj_fwhm_rad", _dp), ("min_fwhm_rad", _dp), ("pa_rad", _dp)]
+
+
+class woden_shapelets_host(C.Structure):
+    _fields_ = [("n", C.c_int), ("n_coeff", C.c_int), ("p_max", C.c_int),
+                ("l", _dp), ("m", _dp), ("s0_jy", _dp), ("alpha", _dp),
+                ("beta1_rad", _dp), ("beta2_rad", _dp), ("pa_rad", _dp), ("uv_basis", _dp),
+                ("coeff_offset", _ip), ("n1", _ip), ("n2", _ip), ("coeff", _dp)]
+
+
+class WodenError(RuntimeError):
+    def __init__(self, status: int, what: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{what}: status {status} ({detail})")
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """Load libwoden_b200.so; raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2005_09316_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    L.woden_create.argtypes = [C.POINTER(_vp), C.c_int]
+    L.woden_destroy.argtypes = [_vp]
+    L.woden_strerror.argtypes = [C.c_int]
+    L.woden_strerror.restype = C.c_char_p
+    L.woden_last_error.argtypes = [_vp]
+    L.woden_last_error.restype = C.c_char_p
+    L.woden_check.argtypes = [_vp]
+    L.woden_set_path.argtypes = [_vp, C.c_int]
+    common = [_vp, C.POINTER(woden_uvw), C.c_int, _vp, _vp, _vp, _vp, C.c_double]
+    tail = [_vp, C.c_int, _vp]
+    L.woden_predict_points.argtypes = common + tail
+    L.woden_predict_gaussians.argtypes = common + [_vp, _vp, _vp] + tail
+    L.woden_predict_shapelets.argtypes = common + [_vp, _vp, _vp, _vp, _vp, C.c_int, C.c_int, _vp, _vp, _vp] + tail
+    L.woden_simulate_host.argtypes = [_vp, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _dp, C.c_double,
+                                      C.POINTER(woden_points_host), C.POINTER(woden_gaussians_host),
+                                      C.POINTER(woden_shapelets_host), _vp, _vp]
+    L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
+    for name in EXPORTS:
+        if name not in ("woden_strerror", "woden_last_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _ptr(t) -> Optional[int]:
+    """Device pointer of a torch tensor (None passes NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> Optional[int]:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+def _hd(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _hdp(a: Optional[np.ndarray]):
+    return None if a is None or a.size == 0 else a.ctypes.data_as(_dp)
+
+
+def _hip(a: Optional[np.ndarray]):
+    return None if a is None or a.size == 0 else a.ctypes.data_as(_ip)
+
+
+class Uvw:
+    """woden_uvw: device u_m, v_m, w_m [T, B] float64 tensors + host channel frequencies."""
+
+    def __init__(self, u_m, v_m, w_m, freqs_hz):
+        import torch
+        for t in (u_m, v_m, w_m):
+            if t.dtype != torch.float64 or t.dim() != 2 or t.shape != u_m.shape:
+                raise ValueError("u_m, v_m, w_m must be float64 [T, B] tensors of one shape")
+        self.tensors = (u_m, v_m, w_m)
+        self.freqs = _hd(freqs_hz)
+        self.T, self.B = int(u_m.shape[0]), int(u_m.shape[1])
+        self.F = int(self.freqs.shape[0])
+        self.c = woden_uvw(self.B, self.T, self.F, _ptr(u_m), _ptr(v_m), _ptr(w_m),
+                           self.freqs.ctypes.data_as(_dp))
+
+    @property
+    def vis_shape(self):
+        return (self.T, self.F, self.B)
+
+
+class Woden:
+    """A woden_ctx.  Methods carry the C entry points' names without the prefix."""
+
+    def __init__(self, device: int = 0):
+        self._L = load()
+        self._ctx = _vp()
+        rc = self._L.woden_create(C.byref(self._ctx), int(device))
+        if rc != WODEN_OK:
+            self._ctx = None
+            raise WodenError(rc, "woden_create", self._L.woden_strerror(rc).decode())
+        self.device = int(device)
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._L.woden_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc: int, what: str):
+        if rc != WODEN_OK:
+            raise WodenError(rc, what, self._L.woden_strerror(rc).decode() + "; "
+                             + self._L.woden_last_error(self._ctx).decode())
+
+    def set_path(self, path: int):
+        self._ck(self._L.woden_set_path(self._ctx, int(path)), "woden_set_path")
+
+    def check(self):
+        self._ck(self._L.woden_check(self._ctx), "woden_check")
+
+    def new_vis(self, uvw: Uvw):
+        import torch
+        return torch.empty(uvw.vis_shape, dtype=torch.complex64, device=uvw.tensors[0].device)
+
+    def predict_points(self, uvw: Uvw, l, m, s0_jy, alpha, ref_freq_hz, vis, accumulate=False, stream=None):
+        n = 0 if l is None else int(l.numel())
+        rc = self._L.woden_predict_points(self._ctx, C.byref(uvw.c), n, _ptr(l), _ptr(m), _ptr(s0_jy),
+                                          _ptr(alpha), float(ref_freq_hz), _ptr(vis), int(bool(accumulate)),
+                                          _stream_handle(stream))
+        self._ck(rc, "woden_predict_points")
+        return vis
+
+    def predict_gaussians(self, uvw: Uvw, l, m, s0_jy, alpha, ref_freq_hz, maj_fwhm_rad, min_fwhm_rad,
+                          pa_rad, vis, accumulate=False, stream=None):
+        n = 0 if l is None else int(l.numel())
+        rc = self._L.woden_predict_gaussians(self._ctx, C.byref(uvw.c), n, _ptr(l), _ptr(m), _ptr(s0_jy),
+                                             _ptr(alpha), float(ref_freq_hz), _ptr(maj_fwhm_rad),
+                                             _ptr(min_fwhm_rad), _ptr(pa_rad), _ptr(vis),
+                                             int(bool(accumulate)), _stream_handle(stream))
+        self._ck(rc, "woden_predict_gaussians")
+        return vis
+
+    def predict_shapelets(self, uvw: Uvw, l, m, s0_jy, alpha, ref_freq_hz, beta1_rad, beta2_rad, pa_rad,
+                          uv_basis, coeff_offset, n_coeff, p_max, n1, n2, coeff, vis, accumulate=False,
+                          stream=None):
+        n = 0 if l is None else int(l.numel())
+        rc = self._L.woden_predict_shapelets(self._ctx, C.byref(uvw.c), n, _ptr(l), _ptr(m), _ptr(s0_jy),
+                                             _ptr(alpha), float(ref_freq_hz), _ptr(beta1_rad), _ptr(beta2_rad),
+                                             _ptr(pa_rad), _ptr(uv_basis), _ptr(coeff_offset), int(n_coeff),
+                                             int(p_max), _ptr(n1), _ptr(n2), _ptr(coeff), _ptr(vis),
+                                             int(bool(accumulate)), _stream_handle(stream))
+        self._ck(rc, "woden_predict_shapelets")
+        return vis
+
+    def simulate_host(self, wl, vis_host: np.ndarray, stream=None) -> np.ndarray:
+        """woden_simulate_host on a generated Workload (host numpy arrays in, complex64 out)."""
+        if vis_host.dtype != np.complex64 or not vis_host.flags.c_contiguous:
+            raise ValueError("vis_host must be C-contiguous complex64")
+        keep = []
+
+        def d(a):
+            a = _hd(a); keep.append(a); return _hdp(a)
+
+        def i(a):
+            a = np.ascontiguousarray(a, dtype=np.int32); keep.append(a); return _hip(a)
+
+        p, g, s = wl.points, wl.gaussians, wl.shapelets
+        cp = woden_points_host(p.n, d(p.l), d(p.m), d(p.s0_jy), d(p.alpha))
+        cg = woden_gaussians_host(g.n, d(g.l), d(g.m), d(g.s0_jy), d(g.alpha),
+                                  d(g.maj_fwhm_rad) if g.n else None, d(g.min_fwhm_rad) if g.n else None,
+                                  d(g.pa_rad) if g.n else None)
+        if s.n:
+            cs = woden_shapelets_host(s.n, int(s.coeff_offset[-1]), int((s.n1 + s.n2).max()),
+                                      d(s.l), d(s.m), d(s.s0_jy), d(s.alpha), d(s.beta1_rad), d(s.beta2_rad),
+                                      d(s.pa_rad), d(s.uv_basis) if s.uv_basis is not None else None,
+                                      i(s.coeff_offset), i(s.n1), i(s.n2), d(s.coeff))
+        else:
+            cs = woden_shapelets_host(0, 0, 0)
+        u, v, w, fr = _hd(wl.u_m), _hd(wl.v_m), _hd(wl.w_m), _hd(wl.freqs_hz)
+        rc = self._L.woden_simulate_host(self._ctx, wl.n_baselines, wl.n_times, wl.n_freqs,
+                                         _hdp(u), _hdp(v), _hdp(w), _hdp(fr), float(wl.ref_freq_hz),
+                                         C.byref(cp), C.byref(cg), C.byref(cs),
+                                         vis_host.ctypes.data_as(_vp), _stream_handle(stream))
+        self._ck(rc, "woden_simulate_host")
+        return vis_host
+
+    def pipe_rate(self, which: str, iters: int = 20000):
+        ops, clk = C.c_double(0.0), C.c_double(0.0)
+        rc = self._L.woden_pipe_rate(self._ctx, PIPES[which], int(iters), C.byref(ops), C.byref(clk))
+        self._ck(rc, "woden_pipe_rate")
+        return ops.value, clk.value
+
+
+class DeviceWorkload:
+    """A generated Workload copied to the GPU once (device-resident inputs for the C-ABI calls)."""
+
+    def __init__(self, wl, device="cuda:0"):
+        import torch
+
+        def t(a, dtype=torch.float64):
+            return None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device=device)
+
+        self.wl = wl
+        self.uvw = Uvw(t(wl.u_m), t(wl.v_m), t(wl.w_m), wl.freqs_hz)
+        self.ref = wl.ref_freq_hz
+        p, g, s = wl.points, wl.gaussians, wl.shapelets
+        self.p = (t(p.l), t(p.m), t(p.s0_jy), t(p.alpha)) if p.n else None
+        self.g = (t(g.l), t(g.m), t(g.s0_jy), t(g.alpha), t(g.maj_fwhm_rad), t(g.min_fwhm_rad),
+                  t(g.pa_rad)) if g.n else None
+        if s.n:
+            self.s = (t(s.l), t(s.m), t(s.s0_jy), t(s.alpha), t(s.beta1_rad), t(s.beta2_rad), t(s.pa_rad),
+                      t(s.uv_basis), t(s.coeff_offset, torch.int32), int(s.coeff_offset[-1]),
+                      int((s.n1 + s.n2).max()), t(s.n1, torch.int32), t(s.n2, torch.int32), t(s.coeff))
+        else:
+            self.s = None
+
+    def predict(self, ctx: Woden, vis=None, stream=None):
+        """The whole hot path: points (overwrite), Gaussians and shapelets (accumulate)."""
+        if vis is None:
+            vis = ctx.new_vis(self.uvw)
+        if self.p is not None:
+            ctx.predict_points(self.uvw, *self.p, self.ref, vis, False, stream)
+        else:
+            ctx.predict_points(self.uvw, None, None, None, None, self.ref, vis, False, stream)
+        if self.g is not None:
+            l, m, s0, al, mj, mn, pa = self.g
+            ctx.predict_gaussians(self.uvw, l, m, s0, al, self.ref, mj, mn, pa, vis, True, stream)
+        if self.s is not None:
+            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = self.s
+            ctx.predict_shapelets(self.uvw, l, m, s0, al, self.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf,
+                                  vis, True, stream)
+        return vis

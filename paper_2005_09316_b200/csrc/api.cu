@@ -1,0 +1,457 @@
+// api.cu -- the C ABI of libwoden_b200.so (include/woden_b200.h): argument validation, the
+// context's grow-only device scratch, the per-call channel table, and kernel sequencing.
+// Host code only; every step of the hot path runs in the kernels it launches.
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/woden_b200.h"
+#include "kernels.h"
+
+using namespace woden;
+
+namespace {
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; cap = 0; }
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+}  // namespace
+
+struct woden_ctx {
+    int device = 0;
+    int path = WODEN_PATH_AUTO;
+    cudaStream_t last_stream = nullptr;
+    std::string last_error;
+    DevBuf geo, flux, tri, chan, err;
+    std::vector<double> chan_freqs;      // frequencies the device channel table was built from
+    int chan_F_pad = 0;
+    ChanTable ch{};
+    // woden_simulate_host staging
+    DevBuf h_uvw, h_comp, h_int, h_vis;
+};
+
+namespace {
+
+constexpr int CHAN_TILE = 16;   // F_pad granularity: lcm of the kernels' channel tiles
+
+int fail_cuda(woden_ctx *ctx, cudaError_t e, const char *where)
+{
+    ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    cudaGetLastError();
+    return WODEN_ERR_CUDA;
+}
+
+#define CU(ctx, call, where)                                                     \
+    do {                                                                         \
+        cudaError_t e__ = (call);                                                \
+        if (e__ != cudaSuccess) return fail_cuda((ctx), e__, (where));           \
+    } while (0)
+
+int check_uvw(const woden_uvw *uvw)
+{
+    if (!uvw || !uvw->u_m || !uvw->v_m || !uvw->w_m || !uvw->freqs_hz) return WODEN_ERR_NULL;
+    if (uvw->n_baselines <= 0 || uvw->n_times <= 0 || uvw->n_freqs <= 0) return WODEN_ERR_DIM;
+    if (uvw->n_freqs > 65535 * 1) return WODEN_ERR_DIM;                  // grid.y of the shapelet kernel
+    for (int f = 0; f < uvw->n_freqs; ++f)
+        if (!(uvw->freqs_hz[f] > 0.0) || !std::isfinite(uvw->freqs_hz[f])) return WODEN_ERR_DIM;
+    return WODEN_OK;
+}
+
+int ensure_err(woden_ctx *ctx, cudaStream_t st)
+{
+    if (!ctx->err.p) {
+        CU(ctx, ctx->err.reserve(sizeof(unsigned int)), "alloc error counter");
+        CU(ctx, cudaMemsetAsync(ctx->err.p, 0, sizeof(unsigned int), st), "clear error counter");
+    }
+    return WODEN_OK;
+}
+
+// Build (or reuse) the device channel table for this frequency list (step S1 constants).
+int ensure_chan(woden_ctx *ctx, const woden_uvw *uvw, cudaStream_t st)
+{
+    const int F = uvw->n_freqs;
+    if ((int)ctx->chan_freqs.size() == F && ctx->chan.p &&
+        std::memcmp(ctx->chan_freqs.data(), uvw->freqs_hz, sizeof(double) * F) == 0)
+        return WODEN_OK;
+    const int F_pad = (F + CHAN_TILE - 1) / CHAN_TILE * CHAN_TILE;
+    const size_t bytes = (size_t)F_pad * (8 + 8 + 4);
+    std::vector<unsigned char> host(bytes, 0);
+    double *s = reinterpret_cast<double *>(host.data());
+    double *nu = s + F_pad;
+    float *ns2 = reinterpret_cast<float *>(nu + F_pad);
+    for (int f = 0; f < F; ++f) {
+        nu[f] = uvw->freqs_hz[f];
+        s[f] = nu[f] / C_LIGHT;
+        ns2[f] = (float)(-(s[f] * s[f]));
+    }
+    int uniform = 0;
+    double ds = 0.0;
+    if (F >= 2) {
+        const double d = uvw->freqs_hz[1] - uvw->freqs_hz[0];
+        uniform = d != 0.0;
+        for (int f = 0; f < F && uniform; ++f)
+            if (std::fabs(uvw->freqs_hz[f] - (uvw->freqs_hz[0] + f * d)) > 1e-9 * std::fabs(d)) uniform = 0;
+        ds = d / C_LIGHT;
+    }
+    ctx->chan_freqs.clear();
+    CU(ctx, ctx->chan.reserve(bytes), "alloc channel table");
+    // pageable source: the runtime stages it before returning, so `host` may die afterwards
+    CU(ctx, cudaMemcpyAsync(ctx->chan.p, host.data(), bytes, cudaMemcpyHostToDevice, st), "upload channel table");
+    ctx->chan_freqs.assign(uvw->freqs_hz, uvw->freqs_hz + F);
+    ctx->chan_F_pad = F_pad;
+    ctx->ch.s = reinterpret_cast<const double *>(ctx->chan.p);
+    ctx->ch.nu = ctx->ch.s + F_pad;
+    ctx->ch.ns2 = reinterpret_cast<const float *>(ctx->ch.nu + F_pad);
+    ctx->ch.F = F;
+    ctx->ch.F_pad = F_pad;
+    ctx->ch.uniform = uniform;
+    ctx->ch.ds = ds;
+    return WODEN_OK;
+}
+
+int zero_or_nothing(woden_ctx *ctx, const woden_uvw *uvw, float *vis, int accumulate, cudaStream_t st)
+{
+    if (!accumulate) {
+        const size_t bytes = (size_t)uvw->n_times * uvw->n_freqs * uvw->n_baselines * 8;
+        CU(ctx, cudaMemsetAsync(vis, 0, bytes, st), "zero-fill vis");
+    }
+    return WODEN_OK;
+}
+
+struct Bind {
+    woden_ctx *ctx;
+    int prev = -1;
+    bool ok = true;
+    explicit Bind(woden_ctx *c) : ctx(c)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        if (prev != c->device && cudaSetDevice(c->device) != cudaSuccess) { ok = false; cudaGetLastError(); }
+    }
+    ~Bind() { if (ok && prev >= 0 && prev != ctx->device) cudaSetDevice(prev); }
+};
+
+int common_checks(woden_ctx *ctx, const woden_uvw *uvw, int n, const double *l, const double *m,
+                  const double *s0, const double *alpha, double ref_freq, const float *vis)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    int rc = check_uvw(uvw);
+    if (rc != WODEN_OK) return rc;
+    if (!vis) return WODEN_ERR_NULL;
+    if (n < 0) return WODEN_ERR_DIM;
+    if (n > 0 && (!l || !m || !s0 || !alpha)) return WODEN_ERR_NULL;
+    if (!(ref_freq > 0.0) || !std::isfinite(ref_freq)) return WODEN_ERR_DIM;
+    if ((long long)uvw->n_times * uvw->n_baselines > (1LL << 38)) return WODEN_ERR_DIM;
+    return WODEN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int woden_create(woden_ctx **out, int cuda_device)
+{
+    if (!out) return WODEN_ERR_NULL;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || cuda_device < 0 || cuda_device >= count) {
+        cudaGetLastError();
+        return WODEN_ERR_CUDA;
+    }
+    woden_ctx *ctx = new (std::nothrow) woden_ctx;
+    if (!ctx) return WODEN_ERR_CUDA;
+    ctx->device = cuda_device;
+    Bind bind(ctx);
+    if (!bind.ok || cudaFree(0) != cudaSuccess) { cudaGetLastError(); delete ctx; return WODEN_ERR_CUDA; }
+    *out = ctx;
+    return WODEN_OK;
+}
+
+int woden_destroy(woden_ctx *ctx)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    {
+        Bind bind(ctx);
+        cudaDeviceSynchronize();
+        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->h_uvw, &ctx->h_comp,
+                          &ctx->h_int, &ctx->h_vis})
+            b->release();
+    }
+    delete ctx;
+    return WODEN_OK;
+}
+
+const char *woden_strerror(int status)
+{
+    switch (status) {
+    case WODEN_OK: return "ok";
+    case WODEN_ERR_NULL: return "a required pointer is NULL";
+    case WODEN_ERR_DIM: return "a size or scalar argument is out of range";
+    case WODEN_ERR_ORDER: return "shapelet order outside 0..WODEN_MAX_ORDER";
+    case WODEN_ERR_CUDA: return "CUDA error (see woden_last_error)";
+    case WODEN_ERR_UNIMPLEMENTED: return "not implemented";
+    case WODEN_ERR_DATA: return "device-side precondition violated (see woden_b200.h)";
+    }
+    return "unknown status";
+}
+
+const char *woden_last_error(const woden_ctx *ctx) { return ctx ? ctx->last_error.c_str() : ""; }
+
+int woden_set_path(woden_ctx *ctx, int path)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    if (path != WODEN_PATH_AUTO && path != WODEN_PATH_GENERAL) return WODEN_ERR_DIM;
+    ctx->path = path;
+    return WODEN_OK;
+}
+
+int woden_check(woden_ctx *ctx)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    CU(ctx, cudaStreamSynchronize(ctx->last_stream), "woden_check sync");
+    if (!ctx->err.p) return WODEN_OK;
+    unsigned int n = 0;
+    CU(ctx, cudaMemcpy(&n, ctx->err.p, sizeof n, cudaMemcpyDeviceToHost), "read error counter");
+    CU(ctx, cudaMemset(ctx->err.p, 0, sizeof n), "clear error counter");
+    return n ? WODEN_ERR_DATA : WODEN_OK;
+}
+
+int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const double *l, const double *m,
+                         const double *s0_jy, const double *alpha, double ref_freq_hz, float *vis,
+                         int accumulate, void *cuda_stream)
+{
+    int rc = common_checks(ctx, uvw, n, l, m, s0_jy, alpha, ref_freq_hz, vis);
+    if (rc != WODEN_OK) return rc;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
+    if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
+    if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
+    const int n_pad = (n + KB - 1) / KB * KB;
+    const int n_ftiles = ctx->ch.F_pad / PG_FT;
+    CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoP)), "alloc geometry");
+    CU(ctx, ctx->flux.reserve((size_t)n_ftiles * n_pad * PG_FT * 4), "alloc flux table");
+    unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
+    launch_pack_points(l, m, n, n_pad, static_cast<GeoP *>(ctx->geo.p), err, st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, static_cast<float *>(ctx->flux.p), err, st);
+    CU(ctx, cudaGetLastError(), "pack points");
+    UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
+    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    CU(ctx, launch_predict_points(d, ctx->ch, static_cast<const GeoP *>(ctx->geo.p),
+                                  static_cast<const float *>(ctx->flux.p), n_pad, reinterpret_cast<float2 *>(vis),
+                                  accumulate ? 1 : 0, walk, st),
+       "predict_points launch");
+    return WODEN_OK;
+}
+
+int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const double *l, const double *m,
+                            const double *s0_jy, const double *alpha, double ref_freq_hz,
+                            const double *maj_fwhm_rad, const double *min_fwhm_rad, const double *pa_rad,
+                            float *vis, int accumulate, void *cuda_stream)
+{
+    int rc = common_checks(ctx, uvw, n, l, m, s0_jy, alpha, ref_freq_hz, vis);
+    if (rc != WODEN_OK) return rc;
+    if (n > 0 && (!maj_fwhm_rad || !min_fwhm_rad || !pa_rad)) return WODEN_ERR_NULL;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
+    if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
+    if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
+    const int n_pad = (n + KB - 1) / KB * KB;
+    const int n_ftiles = ctx->ch.F_pad / PG_FT;
+    CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoG)), "alloc geometry");
+    CU(ctx, ctx->flux.reserve((size_t)n_ftiles * n_pad * PG_FT * 4), "alloc flux table");
+    unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
+    launch_pack_gaussians(l, m, maj_fwhm_rad, min_fwhm_rad, pa_rad, n, n_pad, static_cast<GeoG *>(ctx->geo.p), err,
+                          st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, static_cast<float *>(ctx->flux.p), err, st);
+    CU(ctx, cudaGetLastError(), "pack gaussians");
+    UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
+    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    CU(ctx, launch_predict_gaussians(d, ctx->ch, static_cast<const GeoG *>(ctx->geo.p),
+                                     static_cast<const float *>(ctx->flux.p), n_pad,
+                                     reinterpret_cast<float2 *>(vis), accumulate ? 1 : 0, walk, st),
+       "predict_gaussians launch");
+    return WODEN_OK;
+}
+
+int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const double *l, const double *m,
+                            const double *s0_jy, const double *alpha, double ref_freq_hz,
+                            const double *beta1_rad, const double *beta2_rad, const double *pa_rad,
+                            const double *uv_basis, const int *coeff_offset, int n_coeff, int p_max,
+                            const int *n1, const int *n2, const double *coeff, float *vis, int accumulate,
+                            void *cuda_stream)
+{
+    int rc = common_checks(ctx, uvw, n, l, m, s0_jy, alpha, ref_freq_hz, vis);
+    if (rc != WODEN_OK) return rc;
+    if (n > 0 && (!beta1_rad || !beta2_rad || !pa_rad || !coeff_offset)) return WODEN_ERR_NULL;
+    if (n_coeff < 0) return WODEN_ERR_DIM;
+    if (n_coeff > 0 && (!n1 || !n2 || !coeff)) return WODEN_ERR_NULL;
+    if (p_max < 0 || p_max > WODEN_MAX_ORDER) return WODEN_ERR_ORDER;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
+    if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
+    if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
+    // compile-time order bucket PM >= p_max; pack_coeffs flags any (n1, n2) with n1 + n2 > p_max
+    int PM = shapelet_order_bucket(p_max);
+    if (PM < 0) return WODEN_ERR_ORDER;
+    const size_t tri_floats = (size_t)tri_size(PM);
+    CU(ctx, ctx->geo.reserve((size_t)n * sizeof(GeoS)), "alloc geometry");
+    CU(ctx, ctx->tri.reserve((size_t)n * tri_floats * 4), "alloc coefficient triangles");
+    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n * 4), "alloc flux table");
+    unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
+    launch_pack_shapelets(l, m, beta1_rad, beta2_rad, pa_rad, uv_basis, n, PM, static_cast<GeoS *>(ctx->geo.p), err,
+                          st);
+    launch_pack_coeffs(coeff_offset, n1, n2, coeff, n, n_coeff, p_max, PM, static_cast<float *>(ctx->tri.p), err, st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n, ctx->ch, SH_FT, static_cast<float *>(ctx->flux.p), err, st);
+    CU(ctx, cudaGetLastError(), "pack shapelets");
+    UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
+    CU(ctx, launch_predict_shapelets(d, ctx->ch, static_cast<const GeoS *>(ctx->geo.p),
+                                     static_cast<const float *>(ctx->tri.p),
+                                     static_cast<const float *>(ctx->flux.p), n, PM,
+                                     reinterpret_cast<float2 *>(vis), accumulate ? 1 : 0, st),
+       "predict_shapelets launch");
+    return WODEN_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// sequential sub-allocation of one device arena, 256-byte aligned
+struct Arena {
+    char *base;
+    size_t off = 0;
+    explicit Arena(void *p) : base(static_cast<char *>(p)) {}
+    static size_t pad(size_t b) { return (b + 255) & ~(size_t)255; }
+    template <typename T>
+    T *put(woden_ctx *ctx, const T *host, size_t count, cudaStream_t st, cudaError_t *e)
+    {
+        if (!host || count == 0) return nullptr;
+        T *dst = reinterpret_cast<T *>(base + off);
+        off += pad(count * sizeof(T));
+        if (*e == cudaSuccess) *e = cudaMemcpyAsync(dst, host, count * sizeof(T), cudaMemcpyHostToDevice, st);
+        (void)ctx;
+        return dst;
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freqs, const double *u_m,
+                        const double *v_m, const double *w_m, const double *freqs_hz, double ref_freq_hz,
+                        const woden_points_host *pts, const woden_gaussians_host *gau,
+                        const woden_shapelets_host *shp, float *vis_host, void *cuda_stream)
+{
+    if (!ctx || !u_m || !v_m || !w_m || !freqs_hz || !vis_host) return WODEN_ERR_NULL;
+    if (n_baselines <= 0 || n_times <= 0 || n_freqs <= 0) return WODEN_ERR_DIM;
+    const int np = pts ? pts->n : 0, ng = gau ? gau->n : 0, ns = shp ? shp->n : 0;
+    if (np < 0 || ng < 0 || ns < 0) return WODEN_ERR_DIM;
+    if (np > 0 && (!pts->l || !pts->m || !pts->s0_jy || !pts->alpha)) return WODEN_ERR_NULL;
+    if (ng > 0 && (!gau->l || !gau->m || !gau->s0_jy || !gau->alpha || !gau->maj_fwhm_rad || !gau->min_fwhm_rad ||
+                   !gau->pa_rad))
+        return WODEN_ERR_NULL;
+    if (ns > 0) {
+        if (!shp->l || !shp->m || !shp->s0_jy || !shp->alpha || !shp->beta1_rad || !shp->beta2_rad || !shp->pa_rad ||
+            !shp->coeff_offset)
+            return WODEN_ERR_NULL;
+        if (shp->n_coeff < 0) return WODEN_ERR_DIM;
+        if (shp->n_coeff > 0 && (!shp->n1 || !shp->n2 || !shp->coeff)) return WODEN_ERR_NULL;
+        if (shp->coeff_offset[ns] != shp->n_coeff) return WODEN_ERR_DIM;
+    }
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t TB = (size_t)n_times * n_baselines;
+    const size_t nvis = TB * n_freqs;
+    const size_t nc = ns > 0 ? (size_t)shp->n_coeff : 0;
+    size_t comp_bytes = Arena::pad(8 * (size_t)np) * 4 + Arena::pad(8 * (size_t)ng) * 7 +
+                        Arena::pad(8 * (size_t)ns) * 7 + Arena::pad(48 * (size_t)ns) + Arena::pad(8 * nc) +
+                        Arena::pad(4 * ((size_t)ns + 1)) + 2 * Arena::pad(4 * nc) + 4096;
+    CU(ctx, ctx->h_uvw.reserve(3 * Arena::pad(TB * 8)), "alloc uvw");
+    CU(ctx, ctx->h_comp.reserve(comp_bytes), "alloc components");
+    CU(ctx, ctx->h_vis.reserve(nvis * 8), "alloc vis");
+    cudaError_t e = cudaSuccess;
+    Arena au(ctx->h_uvw.p), ac(ctx->h_comp.p);
+    woden_uvw uvw;
+    uvw.n_baselines = n_baselines; uvw.n_times = n_times; uvw.n_freqs = n_freqs;
+    uvw.u_m = au.put(ctx, u_m, TB, st, &e);
+    uvw.v_m = au.put(ctx, v_m, TB, st, &e);
+    uvw.w_m = au.put(ctx, w_m, TB, st, &e);
+    uvw.freqs_hz = freqs_hz;
+    float *vis = static_cast<float *>(ctx->h_vis.p);
+
+    const double *pl = nullptr, *pm = nullptr, *ps = nullptr, *pa = nullptr;
+    if (np > 0) {
+        pl = ac.put(ctx, pts->l, np, st, &e); pm = ac.put(ctx, pts->m, np, st, &e);
+        ps = ac.put(ctx, pts->s0_jy, np, st, &e); pa = ac.put(ctx, pts->alpha, np, st, &e);
+    }
+    const double *gl = nullptr, *gm = nullptr, *gs = nullptr, *ga = nullptr, *gmj = nullptr, *gmn = nullptr,
+                 *gpa = nullptr;
+    if (ng > 0) {
+        gl = ac.put(ctx, gau->l, ng, st, &e); gm = ac.put(ctx, gau->m, ng, st, &e);
+        gs = ac.put(ctx, gau->s0_jy, ng, st, &e); ga = ac.put(ctx, gau->alpha, ng, st, &e);
+        gmj = ac.put(ctx, gau->maj_fwhm_rad, ng, st, &e); gmn = ac.put(ctx, gau->min_fwhm_rad, ng, st, &e);
+        gpa = ac.put(ctx, gau->pa_rad, ng, st, &e);
+    }
+    const double *sl = nullptr, *sm = nullptr, *ss = nullptr, *sa = nullptr, *sb1 = nullptr, *sb2 = nullptr,
+                 *spa = nullptr, *sM = nullptr, *sc = nullptr;
+    const int *so = nullptr, *sn1 = nullptr, *sn2 = nullptr;
+    if (ns > 0) {
+        sl = ac.put(ctx, shp->l, ns, st, &e); sm = ac.put(ctx, shp->m, ns, st, &e);
+        ss = ac.put(ctx, shp->s0_jy, ns, st, &e); sa = ac.put(ctx, shp->alpha, ns, st, &e);
+        sb1 = ac.put(ctx, shp->beta1_rad, ns, st, &e); sb2 = ac.put(ctx, shp->beta2_rad, ns, st, &e);
+        spa = ac.put(ctx, shp->pa_rad, ns, st, &e);
+        sM = ac.put(ctx, shp->uv_basis, (size_t)6 * ns, st, &e);
+        sc = ac.put(ctx, shp->coeff, nc, st, &e);
+        so = ac.put(ctx, shp->coeff_offset, (size_t)ns + 1, st, &e);
+        sn1 = ac.put(ctx, shp->n1, nc, st, &e); sn2 = ac.put(ctx, shp->n2, nc, st, &e);
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copies");
+
+    int rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
+    if (rc == WODEN_OK && ng > 0)
+        rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, 1, st);
+    if (rc == WODEN_OK && ns > 0)
+        rc = woden_predict_shapelets(ctx, &uvw, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
+                                     shp->p_max, sn1, sn2, sc, vis, 1, st);
+    if (rc != WODEN_OK) return rc;
+    CU(ctx, cudaMemcpyAsync(vis_host, vis, nvis * 8, cudaMemcpyDeviceToHost, st), "device->host vis");
+    CU(ctx, cudaStreamSynchronize(st), "simulate sync");
+    return WODEN_OK;
+}
+
+int woden_pipe_rate(woden_ctx *ctx, int which, int iters, double *thread_ops_per_s, double *sm_clock_hz)
+{
+    if (!ctx || !thread_ops_per_s || !sm_clock_hz) return WODEN_ERR_NULL;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    CU(ctx, run_pipe_rate(which, iters, thread_ops_per_s, sm_clock_hz), "pipe microbenchmark");
+    return WODEN_OK;
+}
+
+}  // extern "C"

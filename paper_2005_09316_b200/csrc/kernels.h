@@ -1,0 +1,49 @@
+// kernels.h -- internal launch interface between api.cu and the kernel translation units.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "layout.h"
+
+namespace woden {
+
+struct UvwDev {
+    const double *u_m, *v_m, *w_m;
+    int B, T, F;
+};
+
+// ---- staging (pack.cu) ------------------------------------------------------------------
+void launch_pack_points(const double *l, const double *m, int n, int n_pad, GeoP *geo,
+                        unsigned int *err, cudaStream_t st);
+void launch_pack_gaussians(const double *l, const double *m, const double *maj, const double *mnr,
+                           const double *pa, int n, int n_pad, GeoG *geo, unsigned int *err,
+                           cudaStream_t st);
+// flux table [n_ftiles][n_pad][FT] = s0 (nu_f/ref)^alpha, zero outside n x F
+void launch_pack_flux(const double *s0, const double *alpha, double ref_freq, int n, int n_pad,
+                      const ChanTable &ch, int FT, float *flux, unsigned int *err, cudaStream_t st);
+void launch_pack_shapelets(const double *l, const double *m, const double *beta1, const double *beta2,
+                           const double *pa, const double *uv_basis, int n, int PM, GeoS *geo,
+                           unsigned int *err, cudaStream_t st);
+// zero `tri` (n * tri_size(PM) floats) then scatter-add sign- and scale-folded coefficients
+void launch_pack_coeffs(const int *coeff_offset, const int *n1, const int *n2, const double *coeff,
+                        int n, int n_coeff, int p_max, int PM, float *tri, unsigned int *err,
+                        cudaStream_t st);
+
+// ---- predict kernels ---------------------------------------------------------------------
+constexpr int PG_FT = 16;        // channels per thread, points / Gaussians
+int pg_smem_bytes(bool gauss);
+cudaError_t launch_predict_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
+                                  int n_pad, float2 *vis, int accumulate, bool walk, cudaStream_t st);
+cudaError_t launch_predict_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo,
+                                     const float *flux, int n_pad, float2 *vis, int accumulate, bool walk,
+                                     cudaStream_t st);
+
+constexpr int SH_FT = 1;         // flux table tile for shapelets: [F][n] layout
+int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or -1
+cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
+                                     const float *flux, int n, int PM, float2 *vis, int accumulate,
+                                     cudaStream_t st);
+
+// ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
+cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
+
+}  // namespace woden

@@ -1,0 +1,235 @@
+// predict_shapelets.cu -- step S6 (+S1, S3, S4, S7) of the hot path for shapelet components
+// (Eq 11 with the envelope of Eq 15-17; basis FT Eq 3, :60).
+//
+// Register path: one thread owns one visibility (b, t, f).  Per
+// shapelet it evaluates the scaled Hermite functions g_p(y) = h_p(y)/lam_p, p = 0..PM, into
+// registers by the two-operation recurrence g_{p+1} = (c_p y) g_p - g_{p-1}, walks g_{n1}(x) on
+// the fly, and contracts the dense coefficient triangle, one FFMA per coefficient, with the
+// coefficients broadcast from shared memory (LDS.128 = 4 coefficients).  The triangle of each
+// shapelet is fetched by one bulk async copy (TMA engine) into shared memory.  The order PM is a
+// compile-time bucket so that every register index and shared-memory offset is static.
+//
+// i^(n1+n2) (reading G3): the sign part (-1)^floor(p/2) of each factor i^p is folded into the
+// stored coefficient by pack.cu, so even n2 add to E, odd n2 to O, and row n1 contributes
+// g_{n1}(x) (E + iO) for even n1, g_{n1}(x) (-O + iE) for odd n1.
+//
+// Underflow (hard part H4): the recurrence starts from 2^64 exp(-x^2/2), formed by one ex2, and
+// its results are scaled back by 2^-64, so orders up to 100 stay accurate where h_0 underflows.
+#include <type_traits>
+
+#include "kernels.h"
+#include "ptx.cuh"
+
+namespace woden {
+namespace {
+
+constexpr int SH_THREADS = 128;
+constexpr double MAGIC23 = 805306368.0;  // 1.5 * 2^29
+constexpr float TWO_PI_F = 6.283185307179586f;
+constexpr float THREE_PI_F = 9.42477796076938f;
+
+// ---- compile-time recurrence constants ----------------------------------------------------
+constexpr double csqrt(double x)
+{
+    double r = x > 1.0 ? x : 1.0;
+    for (int i = 0; i < 64; ++i) r = 0.5 * (r + x / r);
+    return r;
+}
+// lam_0 = lam_1 = 1, lam_{p+1} = sqrt(p/(p+1)) lam_{p-1}
+constexpr double lam_c(int p)
+{
+    double lam = 1.0;
+    for (int q = (p & 1) ? 1 : 0; q + 2 <= p; q += 2) lam *= csqrt((double)(q + 1) / (double)(q + 2));
+    return lam;
+}
+// g_{p+1} = (c_p x) g_p - g_{p-1}
+constexpr double c_rec(int p) { return csqrt(2.0 / (double)(p + 1)) * lam_c(p) / lam_c(p + 1); }
+
+struct RecTable {
+    float c[MAX_ORDER + 1];
+};
+constexpr RecTable make_rec()
+{
+    RecTable t{};
+    for (int p = 0; p <= MAX_ORDER; ++p) t.c[p] = (float)c_rec(p);
+    return t;
+}
+constexpr RecTable REC = make_rec();
+
+struct SParams {
+    const double *u_m, *v_m, *w_m;
+    const GeoS *geo;
+    const float *tri;
+    const float *flux;     // [F][n]
+    const double *chan_s;  // [F_pad]
+    float2 *vis;
+    long long n_bt;
+    int B, F, n, accumulate;
+};
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// g_{Q+1}(y) = (c_Q y) g_Q - g_{Q-1}, Q = 1..PM-1, with compile-time constants
+template <int PM, int Q>
+struct HermY {
+    static __device__ __forceinline__ void run(float (&gy)[PM + 1], float y)
+    {
+        if constexpr (Q < PM) {
+            constexpr float cq = REC.c[Q];
+            gy[Q + 1] = fmaf(cq * y, gy[Q], -gy[Q - 1]);
+            HermY<PM, Q + 1>::run(gy, y);
+        }
+    }
+};
+
+template <int PM, int N1>
+struct Rows {
+    // process rows N1..PM of the triangle; gx0 = g_{N1}(x) * 2^64, gxm = g_{N1-1}(x) * 2^64
+    static __device__ __forceinline__ void run(const float *__restrict__ tri, const float (&gy)[PM + 1], float x,
+                                               float gx0, float gxm, float &re, float &im)
+    {
+        constexpr int LEN = PM - N1 + 1;
+        constexpr int OFF = tri_row_off(PM, N1);
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        const float4 *row = reinterpret_cast<const float4 *>(tri + OFF);
+#pragma unroll
+        for (int q = 0; q < (LEN + 3) / 4; ++q) {
+            const float4 c = row[q];
+            if (4 * q + 0 < LEN) a0 = fmaf(c.x, gy[4 * q + 0], a0);
+            if (4 * q + 1 < LEN) a1 = fmaf(c.y, gy[4 * q + 1], a1);
+            if (4 * q + 2 < LEN) a2 = fmaf(c.z, gy[4 * q + 2], a2);
+            if (4 * q + 3 < LEN) a3 = fmaf(c.w, gy[4 * q + 3], a3);
+        }
+        const float E = a0 + a2, O = a1 + a3;
+        const float gx = gx0 * 5.421010862427522e-20f;     // 2^-64
+        if ((N1 & 1) == 0) { re = fmaf(gx, E, re); im = fmaf(gx, O, im); }
+        else               { re = fmaf(-gx, O, re); im = fmaf(gx, E, im); }
+        if constexpr (N1 < PM) {
+            constexpr float cn = REC.c[N1];
+            const float gx1 = fmaf(cn * x, gx0, -gxm);
+            Rows<PM, N1 + 1>::run(tri, gy, x, gx1, gx0, re, im);
+        }
+    }
+};
+
+template <int PM>
+__global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SParams p)
+{
+    constexpr int TRI = tri_size(PM);
+    __shared__ __align__(128) float tri_s[TRI];
+    __shared__ __align__(8) uint64_t bar;
+
+    const int tid = threadIdx.x;
+    const long long bt = (long long)blockIdx.x * SH_THREADS + tid;
+    const bool valid = bt < p.n_bt;
+    const int f = blockIdx.y;
+
+    if (tid == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
+
+    double u = 0.0, v = 0.0, w = 0.0;
+    if (valid) { u = p.u_m[bt]; v = p.v_m[bt]; w = p.w_m[bt]; }
+    const double s = p.chan_s[f];                  // S1: nu_f / c
+    float acc_re = 0.f, acc_im = 0.f;
+
+    for (int j = 0; j < p.n; ++j) {
+        __syncthreads();                            // previous triangle fully consumed; barrier init visible
+        if (tid == 0) {
+            mbar_arrive_expect_tx(&bar, TRI * 4);
+            bulk_g2s(tri_s, p.tri + (size_t)j * TRI, TRI * 4, &bar);
+        }
+        const GeoS &g = p.geo[j];
+        // S3/S4: phase and phasor
+        const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
+        const unsigned lo = (unsigned)__double2loint(fma(D, s, MAGIC23));
+        const float th = fmaf(__uint_as_float((lo & 0x007fffffu) | 0x3f800000u), TWO_PI_F, -THREE_PI_F);
+        const float cs = -__cosf(th), sn = __sinf(th);          // e^{-2 pi i phi} = cs + i sn
+        // S6 (i)-(ii): x = beta1 K kx', y = beta2 K ky' (Eq 16-17), FP64 then one rounding to FP32
+        const float x = (float)(fma(u, g.X[0], fma(v, g.X[1], w * g.X[2])) * s);
+        const float y = (float)(fma(u, g.Y[0], fma(v, g.Y[1], w * g.Y[2])) * s);
+        const float S = p.flux[(size_t)f * p.n + j];
+
+        // S6 (iii): g_p(y), p = 0..PM, scaled by 2^64 during the recurrence
+        float gy[PM + 1];
+        gy[0] = ex2_approx(fmaf(y * y, -0.7213475204444817f, 64.f));      // 2^64 exp(-y^2/2)
+        {
+            constexpr float c0 = REC.c[0];
+            gy[1] = (c0 * y) * gy[0];
+        }
+        HermY<PM, 1>::run(gy, y);
+#pragma unroll
+        for (int q = 0; q <= PM; ++q) gy[q] *= 5.421010862427522e-20f;    // 2^-64
+        const float gx0 = ex2_approx(fmaf(x * x, -0.7213475204444817f, 64.f));
+
+        mbar_wait(&bar, j & 1);
+        // S6 (iv): xi = sum_{n1} i^{n1} g_{n1}(x) sum_{n2} i^{n2} f'_{n1 n2} g_{n2}(y)
+        float xr = 0.f, xi = 0.f;
+        Rows<PM, 0>::run(tri_s, gy, x, gx0, 0.f, xr, xi);
+        // S7: V += S xi e^{-2 pi i phi}
+        const float zr = xr * cs - xi * sn, zi = xr * sn + xi * cs;
+        acc_re = fmaf(S, zr, acc_re);
+        acc_im = fmaf(S, zi, acc_im);
+    }
+
+    if (valid) {
+        const long long t = bt / p.B;
+        const int b = (int)(bt - t * p.B);
+        float2 *dst = p.vis + ((size_t)t * p.F + f) * p.B + b;
+        float2 val = make_float2(acc_re, acc_im);
+        if (p.accumulate) { const float2 old = *dst; val.x += old.x; val.y += old.y; }
+        *dst = val;
+    }
+}
+
+template <int PM>
+cudaError_t launch_pm(const SParams &p, int F, cudaStream_t st)
+{
+    dim3 grid((unsigned)((p.n_bt + SH_THREADS - 1) / SH_THREADS), (unsigned)F);
+    predict_shapelets_kernel<PM><<<grid, SH_THREADS, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+constexpr int BUCKETS[] = {4, 8, 12, 16, 20, 24, 32, 40, 48, 60, 72, 86, 100};
+
+}  // namespace
+
+int shapelet_order_bucket(int p_max)
+{
+    if (p_max < 0) return -1;
+    for (int b : BUCKETS)
+        if (p_max <= b) return b;
+    return -1;
+}
+
+cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
+                                     const float *flux, int n, int PM, float2 *vis, int accumulate,
+                                     cudaStream_t st)
+{
+    SParams p;
+    p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m;
+    p.geo = geo; p.tri = tri; p.flux = flux; p.chan_s = ch.s; p.vis = vis;
+    p.n_bt = (long long)uvw.T * uvw.B;
+    p.B = uvw.B; p.F = uvw.F; p.n = n; p.accumulate = accumulate;
+    switch (PM) {
+    case 4: return launch_pm<4>(p, uvw.F, st);
+    case 8: return launch_pm<8>(p, uvw.F, st);
+    case 12: return launch_pm<12>(p, uvw.F, st);
+    case 16: return launch_pm<16>(p, uvw.F, st);
+    case 20: return launch_pm<20>(p, uvw.F, st);
+    case 24: return launch_pm<24>(p, uvw.F, st);
+    case 32: return launch_pm<32>(p, uvw.F, st);
+    case 40: return launch_pm<40>(p, uvw.F, st);
+    case 48: return launch_pm<48>(p, uvw.F, st);
+    case 60: return launch_pm<60>(p, uvw.F, st);
+    case 72: return launch_pm<72>(p, uvw.F, st);
+    case 86: return launch_pm<86>(p, uvw.F, st);
+    case 100: return launch_pm<100>(p, uvw.F, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace woden

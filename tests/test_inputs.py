@@ -42,8 +42,8 @@ def test_seeded_determinism_and_hour_angles():
     assert np.array_equal(a.u_m, b.u_m) and np.array_equal(a.points.l, b.points.l)
     # T = 1 => HA = 0 => u = East component of the baseline (w has no Y term at H=0)
     wl = inputs.make_config(2)
-    # hour angles centred on zero: u(t) and u(T-1-t) mirror in the X (sin H) term only
-    assert np.allclose(wl.u_m[0] + wl.u_m[-1], 2 * wl.u_m[0] * 0 + (wl.u_m[0] + wl.u_m[-1]))
+
+
     assert not np.array_equal(wl.u_m[0], wl.u_m[1])
 
 
