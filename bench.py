@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the WODEN hot path (points + Gaussians + shapelets) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5]
+
+One "step" = one pass of the whole hot path over one workload: woden_predict_points
+(overwrite), woden_predict_gaussians and woden_predict_shapelets (accumulate) on config 5
+("Full-band mixed sky", the largest BASELINE.json config; 1.75e8 visibilities, 8000 points,
+2000 Gaussians, 4 shapelets of 861 coefficients), inputs resident in HBM.  Prints ONE JSON
+line (rank 0).  See DESIGN.md "Measurement" for the definitions of every field.
+
+--impl reference times the CPU oracle (oracle/, plain FP64 C, as it stands) on a bounded
+seeded sample of the same workload per step; it is a deliberately slow program, reported as a
+baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2005_09316_b200 import inputs  # noqa: E402
+
+METRIC = "component_x_visibility_evals_per_s"
+UNIT = "evals/s"
+SM_COUNT = 148
+MUFU_LANES_PER_SM = 16          # measured: profiles/pipes_r1.md
+FP32_LANES_PER_SM = 128
+SM_MAX_HZ = 1965e6
+LAUNCHES_PER_STEP = {"points": 3, "gaussians": 3, "shapelets": 5}   # pack + predict kernels
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def workload_counts(wl):
+    nv = wl.n_vis
+    return {
+        "n_vis": nv,
+        "points": nv * wl.points.n,
+        "gaussians": nv * wl.gaussians.n,
+        "shapelets": nv * wl.shapelets.n,
+        "shapelet_coeffs": nv * wl.n_coeff,
+    }
+
+
+def config_dict(wl, extra=None):
+    d = {
+        "workload": f"config {wl.config}: {wl.name}",
+        "n_baselines": wl.n_baselines, "n_times": wl.n_times, "n_freqs": wl.n_freqs,
+        "n_vis": wl.n_vis, "n_points": wl.points.n, "n_gaussians": wl.gaussians.n,
+        "n_shapelets": wl.shapelets.n, "n_shapelet_coeffs": wl.n_coeff,
+        "eval_unit": "one sky component (point, Gaussian or whole shapelet) at one visibility",
+    }
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason sampler running during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        try:
+            rows = [r.strip().split(",") for r in open(self.path) if r.strip()]
+            os.unlink(self.path)
+        except Exception:
+            return out
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); power.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.strip().lower().startswith("active"):
+                        reasons.add(n)
+            except (ValueError, IndexError):
+                continue
+        if sm:
+            busy = sorted(sm)[len(sm) // 2:]          # upper half = samples under load
+            out.update(sm_mhz=float(np.median(busy)), sm_max_mhz=max(mx), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=max(power))
+        return out
+
+
+# ------------------------------------------------------------------------------ reference arm
+def oracle_sample_indices(wl, n, seed_off):
+    rng = np.random.Generator(np.random.PCG64(inputs.SEED_BASE + wl.config + seed_off))
+    return np.sort(rng.integers(0, wl.n_vis, size=n, dtype=np.int64))
+
+
+def time_oracle(wl, n_vis_sample, seed_off):
+    import oracle
+    idx = oracle_sample_indices(wl, n_vis_sample, seed_off)
+    t0 = time.perf_counter()
+    oracle.predict_workload(wl, vis_index=idx)
+    dt = time.perf_counter() - t0
+    comps = wl.points.n + wl.gaussians.n + wl.shapelets.n
+    return n_vis_sample * comps / dt, dt
+
+
+def run_reference(args):
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    wl = inputs.make_config(args.config)
+    cores = len(os.sched_getaffinity(0))
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    n_sample = 1 << 14
+    for i in range(args.warmup):
+        time_oracle(wl, max(256, n_sample // 16), 5000 + i)
+    t_tot, evals = 0.0, 0.0
+    for i in range(args.steps):
+        v, dt = time_oracle(wl, n_sample, 6000 + i)
+        t_tot += dt
+        evals += v * dt
+    value = evals / t_tot
+    sample = (f"{n_sample} seeded random visibilities of config {wl.config} per step, all "
+              f"{wl.points.n + wl.gaussians.n + wl.shapelets.n} components each")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": config_dict(wl, {"sample": sample}),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    from paper_2005_09316_b200 import binding
+
+    rank, world = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1)
+    local = _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
+                         "for the oracle baseline)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # weak scaling: every rank predicts the config's T time steps of one
+    # longer observation with the same sky; shards are disjoint in time, no data-path collective
+    base = inputs.make_config(args.config)
+    T = base.n_times
+    wl = base if world == 1 else inputs.make_config(args.config, t_index0=rank * T, n_times=T,
+                                                     n_times_total=T * world)
+    ctx = binding.Woden(local)
+    ctx.set_path(binding.WODEN_PATH_GENERAL if args.path == "general" else binding.WODEN_PATH_AUTO)
+    dw = binding.DeviceWorkload(wl, device=f"cuda:{local}")
+    vis = ctx.new_vis(dw.uvw)
+    counts = workload_counts(wl)
+    comps = wl.points.n + wl.gaussians.n + wl.shapelets.n
+    evals_per_step = counts["n_vis"] * comps
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    per_type_ms = {"points": [], "gaussians": [], "shapelets": []}
+
+    def step(record):
+        marks = [ev() for _ in range(4)]
+        marks[0].record()
+        if dw.p is not None:
+            ctx.predict_points(dw.uvw, *dw.p, dw.ref, vis, False)
+        else:
+            ctx.predict_points(dw.uvw, None, None, None, None, dw.ref, vis, False)
+        marks[1].record()
+        if dw.g is not None:
+            l, m, s0, al, mj, mn, pa = dw.g
+            ctx.predict_gaussians(dw.uvw, l, m, s0, al, dw.ref, mj, mn, pa, vis, True)
+        marks[2].record()
+        if dw.s is not None:
+            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = dw.s
+            ctx.predict_shapelets(dw.uvw, l, m, s0, al, dw.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf, vis, True)
+        marks[3].record()
+        if record is not None:
+            record.append(marks)
+
+    for _ in range(args.warmup):
+        step(None)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    recs = []
+    e0, e1 = ev(), ev()
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step(recs)
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else {}
+    ms_total = e0.elapsed_time(e1)
+    for marks in recs:
+        for name, a, b in (("points", 0, 1), ("gaussians", 1, 2), ("shapelets", 2, 3)):
+            per_type_ms[name].append(marks[a].elapsed_time(marks[b]))
+    ctx.check()
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / args.steps
+    value = world * evals_per_step / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer C-ABI call (H2D + kernels + D2H inside the timing)
+    vis_host_t = torch.empty(dw.uvw.vis_shape, dtype=torch.complex64, pin_memory=True)
+    vis_host = vis_host_t.numpy()
+    h2d = (3 * wl.u_m.nbytes + 8 * (4 * wl.points.n + 7 * wl.gaussians.n + 13 * wl.shapelets.n)
+           + 16 * wl.n_coeff + 4 * (wl.shapelets.n + 1))
+    d2h = vis_host.nbytes
+    ctx.simulate_host(wl, vis_host)                       # warm-up (allocations)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.simulate_host(wl, vis_host)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * evals_per_step / e2e_s
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- per-type rates and the roofline of the dominant kernel (rank 0)
+    med = {k: float(np.median(v)) if v else None for k, v in per_type_ms.items()}
+    per_type = {}
+    for name, key in (("points", "points"), ("gaussians", "gaussians"), ("shapelets", "shapelets")):
+        if med[name] and counts[key]:
+            per_type[name] = {"evals_per_s": counts[key] / (med[name] * 1e-3), "ms_per_call": med[name]}
+    if "shapelets" in per_type:
+        per_type["shapelets"]["coeff_evals_per_s"] = counts["shapelet_coeffs"] / (med["shapelets"] * 1e-3)
+
+    walk = args.path != "general"        # all configs have uniformly spaced channels
+    mufu_rate, mufu_clk = ctx.pipe_rate("MUFU")
+    fma_rate, _ = ctx.pipe_rate("FFMA")
+    dominant = max((k for k in per_type), key=lambda k: med[k])
+    if dominant == "points":
+        ops = {"walk": ("FP32 FMA pipe: 6 FP32 ops per eval (4 phasor rotation + 2 accumulate)", fma_rate / 6.0),
+               "general": ("MUFU pipe: 2 MUFU (sin, cos) per eval", mufu_rate / 2.0)}
+    elif dominant == "gaussians":
+        ops = {"walk": ("FP32 FMA pipe: 9 FP32 ops per eval (4 rotation + 2 envelope walk + 1 flux*envelope "
+                        "+ 2 accumulate)", fma_rate / 9.0),
+               "general": ("MUFU pipe: 3 MUFU (sin, cos, ex2) per eval", mufu_rate / 3.0)}
+    else:
+        ops = {"walk": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate), "general": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate)}
+    basis, peak = ops["walk" if walk else "general"]
+    ach = (per_type[dominant]["coeff_evals_per_s"] if dominant == "shapelets"
+           else per_type[dominant]["evals_per_s"])
+    roofline = {
+        "bound": "alu", "kernel": f"predict_{dominant}", "achieved": ach / 1e9, "peak": peak / 1e9,
+        "unit": "Gevals/s", "frac": ach / peak, "traffic": None,
+        "peak_basis": basis + f"; pipe rate measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
+        "nominal_mufu_roofline_gevals": SM_COUNT * MUFU_LANES_PER_SM * SM_MAX_HZ / (2 if dominant == "points" else 3) / 1e9,
+    }
+    roofline["frac_of_mufu_roofline"] = ach / 1e9 / roofline["nominal_mufu_roofline_gevals"]
+    # SURVEY.md §8(d) composite roofline time for the whole step at the measured pipe rates
+    t_roof = (counts["points"] / (mufu_rate / 2) + counts["gaussians"] / (mufu_rate / 3)
+              + counts["shapelet_coeffs"] / fma_rate)
+    composite = {"t_roof_ms": 1e3 * t_roof, "t_measured_ms": ms_per_step, "frac": 1e3 * t_roof / ms_per_step,
+                 "definition": "sum_type evals/R_type with R from 2 / 3 MUFU per point / Gaussian eval and "
+                               "1 FFMA per shapelet coefficient (SURVEY.md 8(d)); >1 means the channel-walking "
+                               "path removed MUFU work"}
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        cores = len(os.sched_getaffinity(0))
+        os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+        time_oracle(wl, 2048, 4000)                       # load + build the oracle library
+        n_sample = 1 << 17
+        v, dt = time_oracle(wl, n_sample, 7000)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"{n_sample} seeded random visibilities of config {wl.config}, all {comps} "
+                                  f"components each ({dt:.1f} s)"}
+
+    launches = args.steps * sum(LAUNCHES_PER_STEP[k] for k in ("points", "gaussians", "shapelets")
+                                if counts[k] > 0)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32 accumulate, f64 phase", "data": "synthetic",
+        "config": config_dict(wl, {
+            "path": "auto (channel walking: uniform 80 kHz channels)" if walk else "general",
+            "l2": "no flush: each step writes 1.4 GB of visibilities, 11x the 126 MB L2; component blocks "
+                  "are meant to be L2 resident",
+            "parallelism": "1 GPU" if world == 1 else f"time-sharded x{world}, no collective"}),
+        "per_type": per_type, "roofline": roofline, "composite_roofline": composite,
+        "cpu_baseline": cpu_baseline,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": 1e3 * e2e_s, "call": "woden_simulate_host (pinned host vis buffer)"},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--path", choices=["auto", "general"], default="auto")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
