@@ -174,7 +174,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
-    from paper_2005_09316_b200 import binding
+    from paper_2005_09316_b200 import binding, parallel
 
     rank, world = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1)
     local = _env_int("LOCAL_RANK", 0)
@@ -189,10 +189,7 @@ def run_ours(args):
 
     # weak scaling: every rank predicts the config's T time steps of one
     # longer observation with the same sky; shards are disjoint in time, no data-path collective
-    base = inputs.make_config(args.config)
-    T = base.n_times
-    wl = base if world == 1 else inputs.make_config(args.config, t_index0=rank * T, n_times=T,
-                                                     n_times_total=T * world)
+    wl = parallel.rank_workload(args.config, rank, world, scaling="weak")
     ctx = binding.Woden(local)
     ctx.set_path(binding.WODEN_PATH_GENERAL if args.path == "general" else binding.WODEN_PATH_AUTO)
     dw = binding.DeviceWorkload(wl, device=f"cuda:{local}")
@@ -248,10 +245,7 @@ def run_ours(args):
         for name, a, b in (("points", 0, 1), ("gaussians", 1, 2), ("shapelets", 2, 3)):
             per_type_ms[name].append(marks[a].elapsed_time(marks[b]))
     ctx.check()
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = parallel.max_over_ranks(ms_total, dist, f"cuda:{local}")
     ms_per_step = ms_total / args.steps
     value = world * evals_per_step / (ms_per_step * 1e-3)
 
@@ -268,10 +262,7 @@ def run_ours(args):
         ctx.simulate_host(wl, vis_host)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / args.steps
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = parallel.max_over_ranks(e2e_s, dist, f"cuda:{local}")
     e2e_value = world * evals_per_step / e2e_s
 
     if rank != 0:

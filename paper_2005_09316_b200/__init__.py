@@ -4,4 +4,4 @@
 library (libwoden_b200.so) lazily and fails loudly when it is missing -- there is no CPU
 fallback anywhere in this package.
 """
-__all__ = ["inputs", "binding", "build"]
+__all__ = ["inputs", "binding", "build", "parallel"]

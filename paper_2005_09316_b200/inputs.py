@@ -252,6 +252,13 @@ _OBS = {  # config: (array, T, dt_s, F)
 }
 
 
+def make_config_shape(config: int):
+    """(array name, T, dt_s, F) of config 1..5 without generating it."""
+    if config not in _OBS:
+        raise ValueError(f"config must be 1..5, got {config}")
+    return _OBS[config]
+
+
 def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] = None,
                 n_times: Optional[int] = None) -> Workload:
     """Build config 1..5.  `n_times`/`t_index0`/`n_times_total` select a time shard of a
