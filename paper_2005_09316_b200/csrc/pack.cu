@@ -71,14 +71,18 @@ __global__ void pack_gaussians_kernel(const double *__restrict__ l, const double
     geo[k] = g;
 }
 
-// flux[(ftile * n_pad + k) * FT + j] = s0_k (nu_f / ref)^alpha_k, f = ftile*FT + j  (step S2)
+// flux[(ftile * n_pad + k) * FT + pos] = s0_k (nu_f / ref)^alpha_k  (step S2), where tile position
+// pos holds channel f = ftile*FT + (pos >> 1) + (pos & 1) * FT/2: the two half-tiles are
+// interleaved so that one 64-bit word feeds both lanes of a packed FP32x2 instruction
+// (predict_pg.cu flux_pos); FT == 1 is the plain [F][n] layout.
 __global__ void pack_flux_kernel(const double *__restrict__ s0, const double *__restrict__ alpha, double inv_ref,
                                  int n, int n_pad, const double *__restrict__ nu, int F, int FT, long long total,
                                  float *__restrict__ flux, unsigned int *err)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
-    const int j = (int)(i % FT);
+    const int pos = (int)(i % FT);
+    const int j = FT >= 2 ? (pos >> 1) + (pos & 1) * (FT / 2) : 0;
     const long long r = i / FT;
     const int k = (int)(r % n_pad);
     const int f = (int)(r / n_pad) * FT + j;
