@@ -344,6 +344,23 @@ def run_ours(args):
     return 0
 
 
+def run_pipes(args):
+    """Pipe-rate microbenchmarks (woden_pipe_rate): the measured ALU roofline denominators."""
+    import torch
+    from paper_2005_09316_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --pipes: no CUDA device")
+    ctx = binding.Woden(0)
+    out = {}
+    for name in binding.PIPES:
+        ctx.pipe_rate(name, 2000)
+        best = max((ctx.pipe_rate(name, 20000) for _ in range(3)), key=lambda r: r[0])
+        out[name] = {"thread_ops_per_s": best[0], "sm_clock_hz": best[1],
+                     "per_sm_per_clk": best[0] / SM_COUNT / best[1] if best[1] else None}
+    print(json.dumps({"pipes": out, "sm_count": SM_COUNT}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -353,7 +370,10 @@ def main():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--path", choices=["auto", "general"], default="auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pipes", action="store_true", help="print the measured pipe rates and exit")
     args = ap.parse_args()
+    if args.pipes:
+        return run_pipes(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
