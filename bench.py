@@ -284,14 +284,16 @@ def run_ours(args):
     fma_rate, _ = ctx.pipe_rate("FFMA")
     dominant = max((k for k in per_type), key=lambda k: med[k])
     if dominant == "points":
-        ops = {"walk": ("FP32 FMA pipe: 6 FP32 ops per eval (4 phasor rotation + 2 accumulate)", fma_rate / 6.0),
+        ops = {"walk": ("FP32 FMA pipe: 4 FP32 lane-ops per eval (2 three-term recurrence + 2 accumulate)",
+                        fma_rate / 4.0),
                "general": ("MUFU pipe: 2 MUFU (sin, cos) per eval", mufu_rate / 2.0)}
     elif dominant == "gaussians":
-        ops = {"walk": ("FP32 FMA pipe: 9 FP32 ops per eval (4 rotation + 2 envelope walk + 1 flux*envelope "
-                        "+ 2 accumulate)", fma_rate / 9.0),
+        ops = {"walk": ("FP32 FMA pipe: 7 FP32 lane-ops per eval (2 recurrence + 2 envelope walk + 1 flux*envelope "
+                        "+ 2 accumulate)", fma_rate / 7.0),
                "general": ("MUFU pipe: 3 MUFU (sin, cos, ex2) per eval", mufu_rate / 3.0)}
     else:
-        ops = {"walk": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate), "general": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate)}
+        ops = {"walk": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate),
+               "general": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate)}
     basis, peak = ops["walk" if walk else "general"]
     ach = (per_type[dominant]["coeff_evals_per_s"] if dominant == "shapelets"
            else per_type[dominant]["evals_per_s"])

@@ -46,7 +46,7 @@ struct woden_ctx {
 
 namespace {
 
-constexpr int CHAN_TILE = 16;   // F_pad granularity: lcm of the kernels' channel tiles
+constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
 
 int fail_cuda(woden_ctx *ctx, cudaError_t e, const char *where)
 {
@@ -107,6 +107,10 @@ int ensure_chan(woden_ctx *ctx, const woden_uvw *uvw, cudaStream_t st)
             if (std::fabs(uvw->freqs_hz[f] - (uvw->freqs_hz[0] + f * d)) > 1e-9 * std::fabs(d)) uniform = 0;
         ds = d / C_LIGHT;
     }
+    // the channel-walking kernel seeds its chains at fixed tile positions, which may lie past F in
+    // the last tile: continue the (uniform) grid there; those channels are computed, never stored
+    if (uniform)
+        for (int f = F; f < F_pad; ++f) s[f] = (uvw->freqs_hz[0] + f * (uvw->freqs_hz[1] - uvw->freqs_hz[0])) / C_LIGHT;
     ctx->chan_freqs.clear();
     CU(ctx, ctx->chan.reserve(bytes), "alloc channel table");
     // pageable source: the runtime stages it before returning, so `host` may die afterwards
@@ -245,18 +249,21 @@ int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const doub
     if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
     if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
     const int n_pad = (n + KB - 1) / KB * KB;
-    const int n_ftiles = ctx->ch.F_pad / PG_FT;
+    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoP)), "alloc geometry");
-    CU(ctx, ctx->flux.reserve((size_t)n_ftiles * n_pad * PG_FT * 4), "alloc flux table");
+    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
     unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
     launch_pack_points(l, m, n, n_pad, static_cast<GeoP *>(ctx->geo.p), err, st);
-    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, static_cast<float *>(ctx->flux.p), err, st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, FT, walk, static_cast<float *>(ctx->flux.p), err,
+                     st);
     CU(ctx, cudaGetLastError(), "pack points");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
-    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
-    CU(ctx, launch_predict_points(d, ctx->ch, static_cast<const GeoP *>(ctx->geo.p),
-                                  static_cast<const float *>(ctx->flux.p), n_pad, reinterpret_cast<float2 *>(vis),
-                                  accumulate ? 1 : 0, walk, st),
+    const GeoP *geo = static_cast<const GeoP *>(ctx->geo.p);
+    const float *flux = static_cast<const float *>(ctx->flux.p);
+    float2 *out = reinterpret_cast<float2 *>(vis);
+    CU(ctx, walk ? launch_walk_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st)
+                 : launch_predict_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st),
        "predict_points launch");
     return WODEN_OK;
 }
@@ -277,19 +284,22 @@ int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
     if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
     const int n_pad = (n + KB - 1) / KB * KB;
-    const int n_ftiles = ctx->ch.F_pad / PG_FT;
+    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoG)), "alloc geometry");
-    CU(ctx, ctx->flux.reserve((size_t)n_ftiles * n_pad * PG_FT * 4), "alloc flux table");
+    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
     unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
     launch_pack_gaussians(l, m, maj_fwhm_rad, min_fwhm_rad, pa_rad, n, n_pad, static_cast<GeoG *>(ctx->geo.p), err,
                           st);
-    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, static_cast<float *>(ctx->flux.p), err, st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, FT, walk, static_cast<float *>(ctx->flux.p), err,
+                     st);
     CU(ctx, cudaGetLastError(), "pack gaussians");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
-    const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
-    CU(ctx, launch_predict_gaussians(d, ctx->ch, static_cast<const GeoG *>(ctx->geo.p),
-                                     static_cast<const float *>(ctx->flux.p), n_pad,
-                                     reinterpret_cast<float2 *>(vis), accumulate ? 1 : 0, walk, st),
+    const GeoG *geo = static_cast<const GeoG *>(ctx->geo.p);
+    const float *flux = static_cast<const float *>(ctx->flux.p);
+    float2 *out = reinterpret_cast<float2 *>(vis);
+    CU(ctx, walk ? launch_walk_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st)
+                 : launch_predict_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st),
        "predict_gaussians launch");
     return WODEN_OK;
 }
@@ -325,7 +335,7 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     launch_pack_shapelets(l, m, beta1_rad, beta2_rad, pa_rad, uv_basis, n, PM, static_cast<GeoS *>(ctx->geo.p), err,
                           st);
     launch_pack_coeffs(coeff_offset, n1, n2, coeff, n, n_coeff, p_max, PM, static_cast<float *>(ctx->tri.p), err, st);
-    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n, ctx->ch, SH_FT, static_cast<float *>(ctx->flux.p), err, st);
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n, ctx->ch, SH_FT, false, static_cast<float *>(ctx->flux.p), err, st);
     CU(ctx, cudaGetLastError(), "pack shapelets");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
     CU(ctx, launch_predict_shapelets(d, ctx->ch, static_cast<const GeoS *>(ctx->geo.p),

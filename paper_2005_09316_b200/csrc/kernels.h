@@ -17,9 +17,11 @@ void launch_pack_points(const double *l, const double *m, int n, int n_pad, GeoP
 void launch_pack_gaussians(const double *l, const double *m, const double *maj, const double *mnr,
                            const double *pa, int n, int n_pad, GeoG *geo, unsigned int *err,
                            cudaStream_t st);
-// flux table [n_ftiles][n_pad][FT] = s0 (nu_f/ref)^alpha, zero outside n x F
+// flux table [n_ftiles][n_pad][FT] = s0 (nu_f/ref)^alpha, zero outside n x F; `interleave` stores
+// channel pairs (j, j + FT/2) in adjacent floats (channel-walking kernel)
 void launch_pack_flux(const double *s0, const double *alpha, double ref_freq, int n, int n_pad,
-                      const ChanTable &ch, int FT, float *flux, unsigned int *err, cudaStream_t st);
+                      const ChanTable &ch, int FT, bool interleave, float *flux, unsigned int *err,
+                      cudaStream_t st);
 void launch_pack_shapelets(const double *l, const double *m, const double *beta1, const double *beta2,
                            const double *pa, const double *uv_basis, int n, int PM, GeoS *geo,
                            unsigned int *err, cudaStream_t st);
@@ -29,13 +31,19 @@ void launch_pack_coeffs(const int *coeff_offset, const int *n1, const int *n2, c
                         cudaStream_t st);
 
 // ---- predict kernels ---------------------------------------------------------------------
-constexpr int PG_FT = 16;        // channels per thread, points / Gaussians
-int pg_smem_bytes(bool gauss);
+// general path (predict_pg.cu): any channel list, one sin/cos (+ one exp2) per eval
+constexpr int PG_FT = 16;        // channels per thread
 cudaError_t launch_predict_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, bool walk, cudaStream_t st);
+                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st);
 cudaError_t launch_predict_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo,
-                                     const float *flux, int n_pad, float2 *vis, int accumulate, bool walk,
+                                     const float *flux, int n_pad, float2 *vis, int accumulate,
                                      cudaStream_t st);
+// channel-walking path (predict_walk.cu): equally spaced channels only
+constexpr int WALK_FT = 32;      // channels per thread: two chains of 16
+cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
+                               int n_pad, float2 *vis, int accumulate, cudaStream_t st);
+cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
+                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st);
 
 constexpr int SH_FT = 1;         // flux table tile for shapelets: [F][n] layout
 int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or -1

@@ -71,18 +71,18 @@ __global__ void pack_gaussians_kernel(const double *__restrict__ l, const double
     geo[k] = g;
 }
 
-// flux[(ftile * n_pad + k) * FT + pos] = s0_k (nu_f / ref)^alpha_k  (step S2), where tile position
-// pos holds channel f = ftile*FT + (pos >> 1) + (pos & 1) * FT/2: the two half-tiles are
-// interleaved so that one 64-bit word feeds both lanes of a packed FP32x2 instruction
-// (predict_pg.cu flux_pos); FT == 1 is the plain [F][n] layout.
+// flux[(ftile * n_pad + k) * FT + pos] = s0_k (nu_f / ref)^alpha_k  (step S2).  Plain layout:
+// pos = channel within the tile (FT == 1 is [F][n]).  Interleaved layout (channel-walking kernel):
+// pos holds channel f = ftile*FT + (pos >> 1) + (pos & 1) * FT/2, i.e. the two half-tiles are
+// interleaved so that one 64-bit word feeds both lanes of a packed FP32x2 instruction.
 __global__ void pack_flux_kernel(const double *__restrict__ s0, const double *__restrict__ alpha, double inv_ref,
-                                 int n, int n_pad, const double *__restrict__ nu, int F, int FT, long long total,
-                                 float *__restrict__ flux, unsigned int *err)
+                                 int n, int n_pad, const double *__restrict__ nu, int F, int FT, int interleave,
+                                 long long total, float *__restrict__ flux, unsigned int *err)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     const int pos = (int)(i % FT);
-    const int j = FT >= 2 ? (pos >> 1) + (pos & 1) * (FT / 2) : 0;
+    const int j = interleave ? (pos >> 1) + (pos & 1) * (FT / 2) : pos;
     const long long r = i / FT;
     const int k = (int)(r % n_pad);
     const int f = (int)(r / n_pad) * FT + j;
@@ -201,11 +201,11 @@ void launch_pack_gaussians(const double *l, const double *m, const double *maj, 
 }
 
 void launch_pack_flux(const double *s0, const double *alpha, double ref_freq, int n, int n_pad,
-                      const ChanTable &ch, int FT, float *flux, unsigned int *err, cudaStream_t st)
+                      const ChanTable &ch, int FT, bool interleave, float *flux, unsigned int *err, cudaStream_t st)
 {
     const long long total = (long long)(ch.F_pad / FT) * n_pad * FT;
     pack_flux_kernel<<<blocks_for(total, 256), 256, 0, st>>>(s0, alpha, 1.0 / ref_freq, n, n_pad, ch.nu, ch.F, FT,
-                                                             total, flux, err);
+                                                             interleave ? 1 : 0, total, flux, err);
 }
 
 void launch_pack_shapelets(const double *l, const double *m, const double *beta1, const double *beta2,

@@ -120,6 +120,38 @@ def test_points_ragged_sizes_and_channel_lists(ctx, torch_mod, n, uniform):
     assert err.max() <= TOL
 
 
+@pytest.mark.parametrize("F", [2, 7, 8, 9, 16, 17, 18, 31, 33, 40, 65])
+def test_walking_path_channel_counts_around_the_tile_edges(ctx, torch_mod, F):
+    # equally spaced channels take the channel-walking kernel (32-channel tiles, chains seeded at
+    # tile positions 7 and 23): every F that leaves a seed position past the last channel, and
+    # negative channel steps, must still meet parity for points and Gaussians
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(0)
+    n = 70
+    for step in (40e3, -125e3):
+        u, v, w, _ = _small_case(seed=F, T=2, B=130, F=F)
+        fr = 180e6 + step * np.arange(F)
+        rng = np.random.default_rng(500 + F)
+        l, m = inputs.disk_lm(rng, n, 25.0)
+        s0 = inputs.log_uniform(rng, n, 0.1, 10.0) * rng.choice([-1.0, 1.0], n)
+        al = rng.normal(-0.8, 0.3, n)
+        maj = inputs.log_uniform(rng, n, 0.5, 30.0) * inputs.ARCMIN
+        mnr = maj * rng.uniform(0.1, 1.0, n)
+        pa = rng.uniform(0, np.pi, n)
+        uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+        vis = ctx.new_vis(uvw)
+        args = [_dev(torch, a) for a in (l, m, s0, al)]
+        ctx.predict_points(uvw, *args, 150e6, vis)
+        ctx.predict_gaussians(uvw, *args, 150e6, _dev(torch, maj), _dev(torch, mnr), _dev(torch, pa), vis, True)
+        torch.cuda.synchronize(); ctx.check()
+        ref = oracle.predict_points(u, v, w, fr, l, m, s0, al, 150e6)
+        oracle.predict_gaussians(u, v, w, fr, l, m, s0, al, 150e6, maj, mnr, pa, out=ref, accumulate=True)
+        scale = 2.0 * oracle.tolerance_scale(fr, s0, al, 150e6)
+        err = np.abs(vis.cpu().numpy() - ref) / scale[None, :, None]
+        assert err.max() <= TOL, (F, step, err.max())
+
+
 @pytest.mark.parametrize("uniform", [True, False], ids=["uniform", "irregular"])
 def test_gaussians_ragged_including_zero_width(ctx, torch_mod, uniform):
     from paper_2005_09316_b200 import binding
