@@ -16,7 +16,8 @@ constexpr int PIPE_THREADS = 512;
 constexpr int PIPE_CTAS_PER_SM = 2;
 
 enum { P_FFMA = 0, P_MUFU = 1, P_DFMA = 2, P_I2F = 3, P_LOP3 = 4, P_FFMA2 = 5, P_FFMA_IMM = 6,
-       P_F2F = 7, P_MUFU_EX2 = 8, P_MUFU_FFMA = 9, P_COUNT };
+       P_F2F = 7, P_MUFU_EX2 = 8, P_MUFU_FFMA = 9, P_FFMA_3REG = 10, P_FFMA2_3REG = 11, P_FFMA2_BCAST = 12,
+       P_COUNT };
 
 __device__ __forceinline__ uint64_t globaltimer_ns()
 {
@@ -66,6 +67,46 @@ __global__ void __launch_bounds__(PIPE_THREADS) pipe_kernel(int iters, float see
                     asm("mov.b64 %0, {%1, %2};" : "=l"(z) : "f"(c), "f"(c));
                     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(x) : "l"(x), "l"(y), "l"(z));
                     asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i]), "=f"(a[i + 1]) : "l"(x));
+                }
+        } else if (WHICH == P_FFMA_3REG) {
+            // three distinct register operands per FFMA (no operand shared between neighbours)
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int i = 0; i < CHAINS; i += 2) {
+                    a[i] = fmaf(a[i + 1], __uint_as_float(u[i]), a[i]);
+                    a[i + 1] = fmaf(a[i], __uint_as_float(u[i + 1]), a[i + 1]);
+                }
+        } else if (WHICH == P_FFMA2_3REG) {
+            // x = fma2(y, z, x) with three distinct 64-bit register pairs
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int i = 0; i < CHAINS; i += 4) {
+                    unsigned long long x, y, z, w2;
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(a[i]), "f"(a[i + 1]));
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(a[i + 2]), "f"(a[i + 3]));
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(z) : "r"(u[i]), "r"(u[i + 1]));
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(w2) : "r"(u[i + 2]), "r"(u[i + 3]));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(x) : "l"(y), "l"(z));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(y) : "l"(x), "l"(w2));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i]), "=f"(a[i + 1]) : "l"(x));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i + 2]), "=f"(a[i + 3]) : "l"(y));
+                }
+        } else if (WHICH == P_FFMA2_BCAST) {
+            // x = fma2((c,c), y, x): scalar broadcast operand (SASS R.F32) + two distinct pairs
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int i = 0; i < CHAINS; i += 4) {
+                    unsigned long long x, y, cc;
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(a[i]), "f"(a[i + 1]));
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(a[i + 2]), "f"(a[i + 3]));
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(cc) : "f"(b), "f"(b));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(x) : "l"(cc), "l"(y));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(y) : "l"(cc), "l"(x));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i]), "=f"(a[i + 1]) : "l"(x));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i + 2]), "=f"(a[i + 3]) : "l"(y));
                 }
         } else if (WHICH == P_MUFU) {
 #pragma unroll
@@ -123,7 +164,8 @@ double ops_per_iter(int which)
 {
     switch (which) {
     case P_FFMA: case P_FFMA_IMM: case P_LOP3: return 4.0 * CHAINS;
-    case P_FFMA2: return 4.0 * CHAINS;          // scalar FMAs (2 per f32x2 instruction)
+    case P_FFMA2: case P_FFMA2_3REG: case P_FFMA2_BCAST: return 4.0 * CHAINS;   // scalar FMAs (2 per f32x2)
+    case P_FFMA_3REG: return 4.0 * CHAINS;
     case P_MUFU: case P_MUFU_EX2: case P_I2F: return CHAINS;
     case P_MUFU_FFMA: return CHAINS / 8 * 2;    // MUFU ops; 12 FFMA ride along per 2 MUFU
     case P_DFMA: return CHAINS;                 // 2 x CHAINS/2
@@ -175,6 +217,9 @@ cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double
     case P_F2F: err = run_one<P_F2F>(iters, grid, sink, clk, &ms); break;
     case P_MUFU_EX2: err = run_one<P_MUFU_EX2>(iters, grid, sink, clk, &ms); break;
     case P_MUFU_FFMA: err = run_one<P_MUFU_FFMA>(iters, grid, sink, clk, &ms); break;
+    case P_FFMA_3REG: err = run_one<P_FFMA_3REG>(iters, grid, sink, clk, &ms); break;
+    case P_FFMA2_3REG: err = run_one<P_FFMA2_3REG>(iters, grid, sink, clk, &ms); break;
+    case P_FFMA2_BCAST: err = run_one<P_FFMA2_BCAST>(iters, grid, sink, clk, &ms); break;
     }
     if (err == cudaSuccess) err = cudaMemcpy(hclk, clk, 16, cudaMemcpyDeviceToHost);
     cudaFree(sink); cudaFree(clk);

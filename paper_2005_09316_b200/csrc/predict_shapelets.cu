@@ -18,15 +18,13 @@
 #include <type_traits>
 
 #include "kernels.h"
+#include "phase.cuh"
 #include "ptx.cuh"
 
 namespace woden {
 namespace {
 
 constexpr int SH_THREADS = 128;
-constexpr double MAGIC23 = 805306368.0;  // 1.5 * 2^29
-constexpr float TWO_PI_F = 6.283185307179586f;
-constexpr float THREE_PI_F = 9.42477796076938f;
 
 // ---- compile-time recurrence constants ----------------------------------------------------
 constexpr double csqrt(double x)
@@ -67,13 +65,6 @@ struct SParams {
     int B, F, n, accumulate;
 };
 
-__device__ __forceinline__ float ex2_approx(float x)
-{
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
 // g_{Q+1}(y) = (c_Q y) g_Q - g_{Q-1}, Q = 1..PM-1, with compile-time constants
 template <int PM, int Q>
 struct HermY {
@@ -87,37 +78,55 @@ struct HermY {
     }
 };
 
-template <int PM, int N1>
+template <int PM, int NV, int N1>
 struct Rows {
-    // process rows N1..PM of the triangle; gx0 = g_{N1}(x) * 2^64, gxm = g_{N1-1}(x) * 2^64
-    static __device__ __forceinline__ void run(const float *__restrict__ tri, const float (&gy)[PM + 1], float x,
-                                               float gx0, float gxm, float &re, float &im)
+    // process rows N1..PM of the triangle for NV visibilities; gx0[v] = g_{N1}(x_v) * 2^64,
+    // gxm[v] = g_{N1-1}(x_v) * 2^64.  One LDS.128 (4 coefficients) feeds 4 NV FFMAs.
+    static __device__ __forceinline__ void run(const float *__restrict__ tri, const float (&gy)[NV][PM + 1],
+                                               const float (&x)[NV], float (&gx0)[NV], float (&gxm)[NV],
+                                               float (&re)[NV], float (&im)[NV])
     {
         constexpr int LEN = PM - N1 + 1;
         constexpr int OFF = tri_row_off(PM, N1);
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        float aE[NV], aO[NV], bE[NV], bO[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { aE[v] = 0.f; aO[v] = 0.f; bE[v] = 0.f; bO[v] = 0.f; }
         const float4 *row = reinterpret_cast<const float4 *>(tri + OFF);
 #pragma unroll
         for (int q = 0; q < (LEN + 3) / 4; ++q) {
             const float4 c = row[q];
-            if (4 * q + 0 < LEN) a0 = fmaf(c.x, gy[4 * q + 0], a0);
-            if (4 * q + 1 < LEN) a1 = fmaf(c.y, gy[4 * q + 1], a1);
-            if (4 * q + 2 < LEN) a2 = fmaf(c.z, gy[4 * q + 2], a2);
-            if (4 * q + 3 < LEN) a3 = fmaf(c.w, gy[4 * q + 3], a3);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                if (4 * q + 0 < LEN) aE[v] = fmaf(c.x, gy[v][4 * q + 0], aE[v]);
+                if (4 * q + 1 < LEN) aO[v] = fmaf(c.y, gy[v][4 * q + 1], aO[v]);
+                if (4 * q + 2 < LEN) bE[v] = fmaf(c.z, gy[v][4 * q + 2], bE[v]);
+                if (4 * q + 3 < LEN) bO[v] = fmaf(c.w, gy[v][4 * q + 3], bO[v]);
+            }
         }
-        const float E = a0 + a2, O = a1 + a3;
-        const float gx = gx0 * 5.421010862427522e-20f;     // 2^-64
-        if ((N1 & 1) == 0) { re = fmaf(gx, E, re); im = fmaf(gx, O, im); }
-        else               { re = fmaf(-gx, O, re); im = fmaf(gx, E, im); }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const float E = aE[v] + bE[v], O = aO[v] + bO[v];
+            const float gx = gx0[v] * 5.421010862427522e-20f;     // 2^-64
+            if ((N1 & 1) == 0) { re[v] = fmaf(gx, E, re[v]); im[v] = fmaf(gx, O, im[v]); }
+            else               { re[v] = fmaf(-gx, O, re[v]); im[v] = fmaf(gx, E, im[v]); }
+        }
         if constexpr (N1 < PM) {
             constexpr float cn = REC.c[N1];
-            const float gx1 = fmaf(cn * x, gx0, -gxm);
-            Rows<PM, N1 + 1>::run(tri, gy, x, gx1, gx0, re, im);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const float g1 = fmaf(cn * x[v], gx0[v], -gxm[v]);
+                gxm[v] = gx0[v]; gx0[v] = g1;
+            }
+            Rows<PM, NV, N1 + 1>::run(tri, gy, x, gx0, gxm, re, im);
         }
     }
 };
 
-template <int PM>
+// One thread owns NV visibilities: one (baseline, time) pair at NV consecutive channels.  The
+// coefficient triangle is broadcast from shared memory; a broadcast LDS.128 occupies the shared
+// memory return path for ~2 cycles per SM (profiles/ncu_r1_*.md), i.e. it can feed at most
+// 2 x 4 warp-FFMAs per NV = 1, half of the FMA pipe's rate: NV = 2 lifts that bound.
+template <int PM, int NV>
 __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SParams p)
 {
     constexpr int TRI = tri_size(PM);
@@ -127,14 +136,18 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
     const int tid = threadIdx.x;
     const long long bt = (long long)blockIdx.x * SH_THREADS + tid;
     const bool valid = bt < p.n_bt;
-    const int f = blockIdx.y;
+    const int f0 = blockIdx.y * NV;
 
     if (tid == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
 
     double u = 0.0, v = 0.0, w = 0.0;
     if (valid) { u = p.u_m[bt]; v = p.v_m[bt]; w = p.w_m[bt]; }
-    const double s = p.chan_s[f];                  // S1: nu_f / c
-    float acc_re = 0.f, acc_im = 0.f;
+    double s[NV];                                   // S1: nu_f / c (zero past F: chan_s is padded)
+#pragma unroll
+    for (int i = 0; i < NV; ++i) s[i] = p.chan_s[f0 + i];
+    float acc_re[NV], acc_im[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) { acc_re[i] = 0.f; acc_im[i] = 0.f; }
 
     for (int j = 0; j < p.n; ++j) {
         __syncthreads();                            // previous triangle fully consumed; barrier init visible
@@ -143,53 +156,72 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
             bulk_g2s(tri_s, p.tri + (size_t)j * TRI, TRI * 4, &bar);
         }
         const GeoS &g = p.geo[j];
-        // S3/S4: phase and phasor
+        // S3: phase in metres; S6 (i)-(ii): x = beta1 K kx', y = beta2 K ky' (Eq 16-17) in metres
         const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
-        const unsigned lo = (unsigned)__double2loint(fma(D, s, MAGIC23));
-        const float th = fmaf(__uint_as_float((lo & 0x007fffffu) | 0x3f800000u), TWO_PI_F, -THREE_PI_F);
-        const float cs = -__cosf(th), sn = __sinf(th);          // e^{-2 pi i phi} = cs + i sn
-        // S6 (i)-(ii): x = beta1 K kx', y = beta2 K ky' (Eq 16-17), FP64 then one rounding to FP32
-        const float x = (float)(fma(u, g.X[0], fma(v, g.X[1], w * g.X[2])) * s);
-        const float y = (float)(fma(u, g.Y[0], fma(v, g.Y[1], w * g.Y[2])) * s);
-        const float S = p.flux[(size_t)f * p.n + j];
-
-        // S6 (iii): g_p(y), p = 0..PM, scaled by 2^64 during the recurrence
-        float gy[PM + 1];
-        gy[0] = ex2_approx(fmaf(y * y, -0.7213475204444817f, 64.f));      // 2^64 exp(-y^2/2)
-        {
-            constexpr float c0 = REC.c[0];
-            gy[1] = (c0 * y) * gy[0];
-        }
-        HermY<PM, 1>::run(gy, y);
+        const double xm = fma(u, g.X[0], fma(v, g.X[1], w * g.X[2]));
+        const double ym = fma(u, g.Y[0], fma(v, g.Y[1], w * g.Y[2]));
+        float cs[NV], sn[NV], x[NV], S[NV], gx0[NV], gxm[NV];
+        float gy[NV][PM + 1];
 #pragma unroll
-        for (int q = 0; q <= PM; ++q) gy[q] *= 5.421010862427522e-20f;    // 2^-64
-        const float gx0 = ex2_approx(fmaf(x * x, -0.7213475204444817f, 64.f));
+        for (int i = 0; i < NV; ++i) {
+            // S4: phasor e^{-2 pi i phi} = cs + i sn
+            const float th = theta_from_magic(fma(D, s[i], MAGIC23));
+            cs[i] = -__cosf(th); sn[i] = __sinf(th);
+            x[i] = (float)(xm * s[i]);              // FP64 product, one rounding to FP32
+            const float y = (float)(ym * s[i]);
+            S[i] = (f0 + i < p.F) ? p.flux[(size_t)(f0 + i) * p.n + j] : 0.f;
+            // S6 (iii): g_p(y), p = 0..PM, scaled by 2^64 during the recurrence (hard part H4)
+            gy[i][0] = ex2_approx(fmaf(y * y, -0.7213475204444817f, 64.f));      // 2^64 exp(-y^2/2)
+            if constexpr (PM >= 1) {
+                constexpr float c0 = REC.c[0];
+                gy[i][1] = (c0 * y) * gy[i][0];
+                HermY<PM, 1>::run(gy[i], y);
+            }
+#pragma unroll
+            for (int q = 0; q <= PM; ++q) gy[i][q] *= 5.421010862427522e-20f;    // 2^-64
+            gx0[i] = ex2_approx(fmaf(x[i] * x[i], -0.7213475204444817f, 64.f));
+            gxm[i] = 0.f;
+        }
 
         mbar_wait(&bar, j & 1);
         // S6 (iv): xi = sum_{n1} i^{n1} g_{n1}(x) sum_{n2} i^{n2} f'_{n1 n2} g_{n2}(y)
-        float xr = 0.f, xi = 0.f;
-        Rows<PM, 0>::run(tri_s, gy, x, gx0, 0.f, xr, xi);
+        float xr[NV], xi[NV];
+#pragma unroll
+        for (int i = 0; i < NV; ++i) { xr[i] = 0.f; xi[i] = 0.f; }
+        Rows<PM, NV, 0>::run(tri_s, gy, x, gx0, gxm, xr, xi);
         // S7: V += S xi e^{-2 pi i phi}
-        const float zr = xr * cs - xi * sn, zi = xr * sn + xi * cs;
-        acc_re = fmaf(S, zr, acc_re);
-        acc_im = fmaf(S, zi, acc_im);
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            const float zr = xr[i] * cs[i] - xi[i] * sn[i], zi = xr[i] * sn[i] + xi[i] * cs[i];
+            acc_re[i] = fmaf(S[i], zr, acc_re[i]);
+            acc_im[i] = fmaf(S[i], zi, acc_im[i]);
+        }
     }
 
     if (valid) {
         const long long t = bt / p.B;
         const int b = (int)(bt - t * p.B);
-        float2 *dst = p.vis + ((size_t)t * p.F + f) * p.B + b;
-        float2 val = make_float2(acc_re, acc_im);
-        if (p.accumulate) { const float2 old = *dst; val.x += old.x; val.y += old.y; }
-        *dst = val;
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            if (f0 + i < p.F) {
+                float2 *dst = p.vis + ((size_t)t * p.F + f0 + i) * p.B + b;
+                float2 val = make_float2(acc_re[i], acc_im[i]);
+                if (p.accumulate) { const float2 old = *dst; val.x += old.x; val.y += old.y; }
+                *dst = val;
+            }
+        }
     }
 }
+
+// visibilities per thread: registers hold NV (PM + 1) Hermite values
+constexpr int nv_for(int PM) { return PM <= 16 ? 4 : (PM <= 40 ? 2 : 1); }
 
 template <int PM>
 cudaError_t launch_pm(const SParams &p, int F, cudaStream_t st)
 {
-    dim3 grid((unsigned)((p.n_bt + SH_THREADS - 1) / SH_THREADS), (unsigned)F);
-    predict_shapelets_kernel<PM><<<grid, SH_THREADS, 0, st>>>(p);
+    constexpr int NV = nv_for(PM);
+    dim3 grid((unsigned)((p.n_bt + SH_THREADS - 1) / SH_THREADS), (unsigned)((F + NV - 1) / NV));
+    predict_shapelets_kernel<PM, NV><<<grid, SH_THREADS, 0, st>>>(p);
     return cudaGetLastError();
 }
 
