@@ -13,8 +13,9 @@
 // stored coefficient by pack.cu, so even n2 add to E, odd n2 to O, and row n1 contributes
 // g_{n1}(x) (E + iO) for even n1, g_{n1}(x) (-O + iE) for odd n1.
 //
-// Underflow (hard part H4): the recurrence starts from 2^64 exp(-x^2/2), formed by one ex2, and
-// its results are scaled back by 2^-64, so orders up to 100 stay accurate where h_0 underflows.
+// Underflow (hard part H4): both recurrences start from 2^64 exp(-x^2/2), formed by one ex2, so
+// orders up to 100 stay accurate where h_0 underflows; g(x) is scaled back by 2^-64 per row and
+// the row sums (which carry g(y)'s 2^64) once per shapelet.
 #include <type_traits>
 
 #include "kernels.h"
@@ -88,24 +89,30 @@ struct Rows {
     {
         constexpr int LEN = PM - N1 + 1;
         constexpr int OFF = tri_row_off(PM, N1);
-        float aE[NV], aO[NV], bE[NV], bO[NV];
+        // NV >= 2 already gives 2 NV independent FFMA chains; NV == 1 splits each into two
+        constexpr int NS = NV >= 2 ? 1 : 2;
+        float aE[NV][NS], aO[NV][NS];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) { aE[v] = 0.f; aO[v] = 0.f; bE[v] = 0.f; bO[v] = 0.f; }
+        for (int v = 0; v < NV; ++v)
+#pragma unroll
+            for (int h = 0; h < NS; ++h) { aE[v][h] = 0.f; aO[v][h] = 0.f; }
         const float4 *row = reinterpret_cast<const float4 *>(tri + OFF);
 #pragma unroll
         for (int q = 0; q < (LEN + 3) / 4; ++q) {
             const float4 c = row[q];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                if (4 * q + 0 < LEN) aE[v] = fmaf(c.x, gy[v][4 * q + 0], aE[v]);
-                if (4 * q + 1 < LEN) aO[v] = fmaf(c.y, gy[v][4 * q + 1], aO[v]);
-                if (4 * q + 2 < LEN) bE[v] = fmaf(c.z, gy[v][4 * q + 2], bE[v]);
-                if (4 * q + 3 < LEN) bO[v] = fmaf(c.w, gy[v][4 * q + 3], bO[v]);
+                if (4 * q + 0 < LEN) aE[v][0] = fmaf(c.x, gy[v][4 * q + 0], aE[v][0]);
+                if (4 * q + 1 < LEN) aO[v][0] = fmaf(c.y, gy[v][4 * q + 1], aO[v][0]);
+                if (4 * q + 2 < LEN) aE[v][NS - 1] = fmaf(c.z, gy[v][4 * q + 2], aE[v][NS - 1]);
+                if (4 * q + 3 < LEN) aO[v][NS - 1] = fmaf(c.w, gy[v][4 * q + 3], aO[v][NS - 1]);
             }
         }
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
-            const float E = aE[v] + bE[v], O = aO[v] + bO[v];
+            const float E = NS == 2 ? aE[v][0] + aE[v][NS - 1] : aE[v][0];
+            const float O = NS == 2 ? aO[v][0] + aO[v][NS - 1] : aO[v][0];
+            // gx0 carries 2^64 (hard part H4); gy's 2^64 is undone once per shapelet by the caller
             const float gx = gx0[v] * 5.421010862427522e-20f;     // 2^-64
             if ((N1 & 1) == 0) { re[v] = fmaf(gx, E, re[v]); im[v] = fmaf(gx, O, im[v]); }
             else               { re[v] = fmaf(-gx, O, re[v]); im[v] = fmaf(gx, E, im[v]); }
@@ -177,8 +184,6 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
                 gy[i][1] = (c0 * y) * gy[i][0];
                 HermY<PM, 1>::run(gy[i], y);
             }
-#pragma unroll
-            for (int q = 0; q <= PM; ++q) gy[i][q] *= 5.421010862427522e-20f;    // 2^-64
             gx0[i] = ex2_approx(fmaf(x[i] * x[i], -0.7213475204444817f, 64.f));
             gxm[i] = 0.f;
         }
@@ -192,6 +197,7 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
         // S7: V += S xi e^{-2 pi i phi}
 #pragma unroll
         for (int i = 0; i < NV; ++i) {
+            xr[i] *= 5.421010862427522e-20f; xi[i] *= 5.421010862427522e-20f;      // gy's 2^64
             const float zr = xr[i] * cs[i] - xi[i] * sn[i], zi = xr[i] * sn[i] + xi[i] * cs[i];
             acc_re[i] = fmaf(S[i], zr, acc_re[i]);
             acc_im[i] = fmaf(S[i], zi, acc_im[i]);

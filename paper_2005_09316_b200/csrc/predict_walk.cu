@@ -11,7 +11,7 @@
 // Per (thread, component):
 //   D = u_m l + v_m m + w_m (n-1)                       FP64 metres (3 FP64 ops, hard part H1)
 //   seeds: q = exp(i theta) at chain position J0 = 7 of both chains by true sin/cos of the FP64
-//          phase reduced to its fraction (4 MUFU), w = exp(i delta), delta = 2 pi D dnu/c (2 MUFU);
+//          phase reduced to its fraction as Q0.32 (4 MUFU), w = exp(i delta), delta = 2 pi D dnu/c (2 MUFU);
 //          position J0 + 1 by one complex rotation with w.
 //   walk : with channels nu_0 + j dnu the real and imaginary parts of q_j each obey
 //          x_{j+1} = 2 cos(delta) x_j - x_{j-1}: ONE FMA per real number per channel.  The chain
@@ -23,8 +23,8 @@
 //   scalars +c / -c, and s_j is applied once per visibility in the epilogue.
 //   Gaussians: xi_j = exp2(-Q s_j^2), s_j = nu_j / c, is walked both ways by the second-order
 //   multiplicative recurrence xi_{j+1} = xi_j rho_j, rho_{j+1} = rho_j qq (7 MUFU seeds).
-//   The kernel accumulates sum S q with q = exp(+i theta), theta = 2 pi (frac(phi) - 1/2);
-//   exp(-2 pi i phi) = -conj(q), so the epilogue stores (-re, im).
+//   The kernel accumulates sum S q with q = exp(+i theta), theta = 2 pi frac(phi);
+//   exp(-2 pi i phi) = conj(q), so the epilogue stores (re, -im).
 //
 // Staging: component geometry (32 / 48 B) and the 32 precomputed fluxes S_k(nu_f) of the tile are
 // fetched in blocks of KB = 64 components by 1-D bulk async copies (TMA engine, SASS UBLKCP) into a
@@ -69,13 +69,18 @@ struct Seed {
 
 template <bool GAUSS, typename Geo>
 __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, double w, float uf, float vf,
-                                          double sfA, double sfB, double ds, Seed<GAUSS> &sd)
+                                          double sfA, double ds, Seed<GAUSS> &sd)
 {
     // S3: D = u l + v m + w (n-1), FP64 metres
     const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
-    const float thA = theta_from_magic(fma(D, sfA, MAGIC23));
-    const float thB = theta_from_magic(fma(D, sfB, MAGIC23));
-    const float thd = theta_from_q32(fma(D, ds, MAGIC32));
+    // frac(phase) as signed Q0.32 (low word of phase + 1.5*2^20): chain A's seed and the channel
+    // step by one DFMA each; chain B's seed, WH channels up, by integer arithmetic (wraps mod 1 turn)
+    const unsigned qA = (unsigned)__double2loint(fma(D, sfA, MAGIC32));
+    const unsigned qd = (unsigned)__double2loint(fma(D, ds, MAGIC32));
+    const unsigned qB = qA + (unsigned)WH * qd;
+    const float thA = (float)(int)qA * Q32_TO_RAD;
+    const float thB = (float)(int)qB * Q32_TO_RAD;
+    const float thd = (float)(int)qd * Q32_TO_RAD;
     sd.cA = __cosf(thA); sd.sA = __sinf(thA);
     sd.cB = __cosf(thB); sd.sB = __sinf(thB);
     sd.wr = __cosf(thd); sd.wi = __sinf(thd);
@@ -173,12 +178,12 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
         const unsigned char *fl = smem + s * STAGE_BYTES + GEO_BYTES;
 
         Seed<GAUSS> sd;
-        make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, sfB, ds, sd);
+        make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, ds, sd);
 #pragma unroll 1
         for (int k = 0; k < KB; ++k) {
             // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
             Seed<GAUSS> nx;
-            make_seed<GAUSS>(g[k + 1 < KB ? k + 1 : k], u, v, w, uf, vf, sfA, sfB, ds, nx);
+            make_seed<GAUSS>(g[k + 1 < KB ? k + 1 : k], u, v, w, uf, vf, sfA, ds, nx);
 
             const ulonglong2 *fl2 = reinterpret_cast<const ulonglong2 *>(fl + (size_t)k * FT * 4);
             const float cf = sd.wr + sd.wr;                    // c = 2 cos(delta)
@@ -256,7 +261,7 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
         if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
     }
 
-    // S7: exp(-2 pi i phi) = -conj(q): V = (-re, im); coalesced float2 stores along b
+    // S7: exp(-2 pi i phi) = conj(q): V = (re, -im); coalesced float2 stores along b
     if (valid) {
         const long long t = bt / p.B;
         const int b = (int)(bt - t * p.B);
@@ -271,7 +276,7 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
             if (walk_neg(j % H)) { re = -re; im = -im; }      // s_j of the recurrence
             if (f < p.F) {
                 float2 *dst = p.vis + ((size_t)t * p.F + f) * p.B + b;
-                float2 val = make_float2(-re, im);
+                float2 val = make_float2(re, -im);
                 if (p.accumulate) { const float2 old = *dst; val.x += old.x; val.y += old.y; }
                 *dst = val;
             }
