@@ -38,6 +38,9 @@ MUFU_LANES_PER_SM = 16          # measured: profiles/pipes_r1.md
 FP32_LANES_PER_SM = 128
 SM_MAX_HZ = 1965e6
 LAUNCHES_PER_STEP = {"points": 3, "gaussians": 3, "shapelets": 5}   # pack + predict kernels
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on config 5 (profiles/ncu_r1_kernels.md)
+NCU_DRAM_BYTES = {("points", "walk"): 158166016 + 1345318912, ("gaussians", "walk"): 1536168960 + 1339894272,
+                  ("shapelets", "walk"): 1419681792 + 1340600320, ("shapelets", "general"): 1419681792 + 1340600320}
 
 
 def _env_int(name, default):
@@ -297,9 +300,16 @@ def run_ours(args):
     basis, peak = ops["walk" if walk else "general"]
     ach = (per_type[dominant]["coeff_evals_per_s"] if dominant == "shapelets"
            else per_type[dominant]["evals_per_s"])
+    # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r1_kernels.md):
+    # the visibility buffer once, plus the component blocks that miss L2
+    traffic = NCU_DRAM_BYTES.get((dominant, "walk" if walk else "general")) if args.config == 5 else None
+    ffma2_3reg, _ = ctx.pipe_rate("FFMA2_3REG")
     roofline = {
         "bound": "alu", "kernel": f"predict_{dominant}", "achieved": ach / 1e9, "peak": peak / 1e9,
-        "unit": "Gevals/s", "frac": ach / peak, "traffic": None,
+        "unit": "Gevals/s", "frac": ach / peak, "traffic": traffic,
+        "operand_delivery": {"ffma2_three_fresh_pairs_fma_per_s": ffma2_3reg, "ffma_reused_operands_fma_per_s": fma_rate,
+                             "note": "register file feeds ~2 operands/clk/sub-partition: an FMA with three fresh "
+                                     "register operands runs at 2/3 of the pipe rate (DESIGN.md section 7)"},
         "peak_basis": basis + f"; pipe rate measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
         "nominal_mufu_roofline_gevals": SM_COUNT * MUFU_LANES_PER_SM * SM_MAX_HZ / (2 if dominant == "points" else 3) / 1e9,
     }
