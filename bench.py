@@ -373,6 +373,58 @@ def run_pipes(args):
     return 0
 
 
+def run_truncation(args):
+    """GPU time against the kept fraction f_comp (section 5.3, Eq 23-24; the shape of Fig 7's
+    timing panels): config 4's MS-CLEAN-like point/Gaussian model and its two-lobe shapelet model."""
+    import torch
+    from paper_2005_09316_b200 import binding, truncate
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --truncation: no CUDA device")
+    wl = inputs.make_config(4)
+    ctx = binding.Woden(0)
+    uvw = binding.Uvw(*(torch.as_tensor(a, device="cuda:0") for a in (wl.u_m, wl.v_m, wl.w_m)), wl.freqs_hz)
+    vis = ctx.new_vis(uvw)
+    dev = lambda a, dt=torch.float64: torch.as_tensor(np.ascontiguousarray(a), dtype=dt, device="cuda:0")
+    w_sh = truncate.shapelet_basis_weights(wl.shapelets)
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(max(3, args.steps)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+
+    rows = []
+    for f in (1.0, 0.8, 0.6, 0.4, 0.2, 0.1):
+        p, g = truncate.truncate_components(wl.points, f), truncate.truncate_components(wl.gaussians, f)
+        s = truncate.truncate_shapelets(wl.shapelets, f, w_sh)
+        dp = [dev(a) for a in (p.l, p.m, p.s0_jy, p.alpha)]
+        dg = [dev(a) for a in (g.l, g.m, g.s0_jy, g.alpha, g.maj_fwhm_rad, g.min_fwhm_rad, g.pa_rad)]
+        ds_ = [dev(a) for a in (s.l, s.m, s.s0_jy, s.alpha, s.beta1_rad, s.beta2_rad, s.pa_rad, s.uv_basis)]
+        di = [dev(a, torch.int32) for a in (s.coeff_offset, s.n1, s.n2)]
+        dc = dev(s.coeff)
+        pmax = int((s.n1 + s.n2).max())
+
+        def clean():
+            ctx.predict_points(uvw, *dp, wl.ref_freq_hz, vis, False)
+            ctx.predict_gaussians(uvw, *dg[:4], wl.ref_freq_hz, *dg[4:], vis, True)
+
+        def shp():
+            ctx.predict_shapelets(uvw, *ds_[:4], wl.ref_freq_hz, *ds_[4:], di[0], int(s.coeff.size), pmax,
+                                  di[1], di[2], dc, vis, False)
+
+        rows.append({"f_comp": f, "msclean_components": p.n + g.n, "msclean_ms": timed(clean),
+                     "shapelet_basis_functions": int(s.coeff.size), "shapelet_p_max": pmax, "shapelet_ms": timed(shp)})
+    ctx.check()
+    print(json.dumps({"truncation": rows, "workload": "config 4 (8128 baselines x 14 steps x 384 channels)",
+                      "note": "one launch set per model; medians of CUDA-event times"}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -383,9 +435,13 @@ def main():
     ap.add_argument("--path", choices=["auto", "general"], default="auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipes", action="store_true", help="print the measured pipe rates and exit")
+    ap.add_argument("--truncation", action="store_true",
+                    help="GPU time vs kept fraction of components (PAPER.md section 5.3) and exit")
     args = ap.parse_args()
     if args.pipes:
         return run_pipes(args)
+    if args.truncation:
+        return run_truncation(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -42,10 +42,13 @@ struct woden_ctx {
     ChanTable ch{};
     // woden_simulate_host staging
     DevBuf h_uvw, h_comp, h_int, h_vis;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t chunk_done[8] = {};
 };
 
 namespace {
 
+constexpr int SIM_CHUNKS = 8;   // time chunks of woden_simulate_host (compute / copy-back overlap)
 constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
 
 int fail_cuda(woden_ctx *ctx, cudaError_t e, const char *where)
@@ -190,6 +193,10 @@ int woden_destroy(woden_ctx *ctx)
     {
         Bind bind(ctx);
         cudaDeviceSynchronize();
+        if (ctx->copy_stream) {
+            cudaStreamDestroy(ctx->copy_stream);
+            for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
+        }
         for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->h_uvw, &ctx->h_comp,
                           &ctx->h_int, &ctx->h_vis})
             b->release();
@@ -327,7 +334,7 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     // compile-time order bucket PM >= p_max; pack_coeffs flags any (n1, n2) with n1 + n2 > p_max
     int PM = shapelet_order_bucket(p_max);
     if (PM < 0) return WODEN_ERR_ORDER;
-    const size_t tri_floats = (size_t)tri_size(PM);
+    const size_t tri_floats = (size_t)tri_stride(PM);
     CU(ctx, ctx->geo.reserve((size_t)n * sizeof(GeoS)), "alloc geometry");
     CU(ctx, ctx->tri.reserve((size_t)n * tri_floats * 4), "alloc coefficient triangles");
     CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n * 4), "alloc flux table");
@@ -338,9 +345,12 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n, ctx->ch, SH_FT, false, static_cast<float *>(ctx->flux.p), err, st);
     CU(ctx, cudaGetLastError(), "pack shapelets");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
+    // truncated models: when under 3/4 of the order bucket's triangle is listed, take
+    // the kernel variant that skips empty 4-coefficient chunks (decided from the list length alone)
+    const bool sparse = (double)n_coeff < 0.75 * (double)n * (double)((PM + 1) * (PM + 2) / 2);
     CU(ctx, launch_predict_shapelets(d, ctx->ch, static_cast<const GeoS *>(ctx->geo.p),
                                      static_cast<const float *>(ctx->tri.p),
-                                     static_cast<const float *>(ctx->flux.p), n, PM,
+                                     static_cast<const float *>(ctx->flux.p), n, PM, sparse,
                                      reinterpret_cast<float2 *>(vis), accumulate ? 1 : 0, st),
        "predict_shapelets launch");
     return WODEN_OK;
@@ -443,15 +453,46 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     }
     if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copies");
 
-    int rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
-    if (rc == WODEN_OK && ng > 0)
+    // Time steps are independent (Eq 9 sums over components only): the last predictor runs in chunks
+    // of time steps and each finished chunk is copied back on a second stream meanwhile.
+    if (!ctx->copy_stream) {
+        CU(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "create copy stream");
+        for (cudaEvent_t &ev : ctx->chunk_done) CU(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "create event");
+    }
+    // All types but the last run over the whole observation in one launch (no tail loss); only
+    // the last one is chunked, and its chunks' copies hide behind the chunks that follow.
+    const int last = ns > 0 ? 2 : (ng > 0 ? 1 : 0);
+    int rc = WODEN_OK;
+    if (last > 0) rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
+    if (rc == WODEN_OK && last > 1 && ng > 0)
         rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, 1, st);
-    if (rc == WODEN_OK && ns > 0)
-        rc = woden_predict_shapelets(ctx, &uvw, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
-                                     shp->p_max, sn1, sn2, sc, vis, 1, st);
-    if (rc != WODEN_OK) return rc;
-    CU(ctx, cudaMemcpyAsync(vis_host, vis, nvis * 8, cudaMemcpyDeviceToHost, st), "device->host vis");
+    const int n_chunks = n_times < SIM_CHUNKS ? n_times : SIM_CHUNKS;
+    for (int c = 0; c < n_chunks && rc == WODEN_OK; ++c) {
+        const int t0 = (int)((long long)n_times * c / n_chunks), t1 = (int)((long long)n_times * (c + 1) / n_chunks);
+        woden_uvw part = uvw;
+        part.n_times = t1 - t0;
+        part.u_m = uvw.u_m + (size_t)t0 * n_baselines;
+        part.v_m = uvw.v_m + (size_t)t0 * n_baselines;
+        part.w_m = uvw.w_m + (size_t)t0 * n_baselines;
+        const size_t off = (size_t)t0 * n_freqs * n_baselines, cnt = (size_t)(t1 - t0) * n_freqs * n_baselines;
+        float *vc = vis + 2 * off;
+        if (last == 0)
+            rc = woden_predict_points(ctx, &part, np, pl, pm, ps, pa, ref_freq_hz, vc, 0, st);
+        else if (last == 1)
+            rc = woden_predict_gaussians(ctx, &part, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vc, 1, st);
+        else
+            rc = woden_predict_shapelets(ctx, &part, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
+                                         shp->p_max, sn1, sn2, sc, vc, 1, st);
+        if (rc != WODEN_OK) break;
+        CU(ctx, cudaEventRecord(ctx->chunk_done[c], st), "record chunk");
+        CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->chunk_done[c], 0), "wait chunk");
+        CU(ctx, cudaMemcpyAsync(vis_host + 2 * off, vc, cnt * 8, cudaMemcpyDeviceToHost, ctx->copy_stream),
+           "device->host vis");
+    }
+    if (rc != WODEN_OK) { cudaStreamSynchronize(st); cudaStreamSynchronize(ctx->copy_stream); return rc; }
     CU(ctx, cudaStreamSynchronize(st), "simulate sync");
+    CU(ctx, cudaStreamSynchronize(ctx->copy_stream), "simulate copy sync");
+    ctx->last_stream = st;
     return WODEN_OK;
 }
 

@@ -48,7 +48,7 @@ cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const 
 constexpr int SH_FT = 1;         // flux table tile for shapelets: [F][n] layout
 int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or -1
 cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
-                                     const float *flux, int n, int PM, float2 *vis, int accumulate,
+                                     const float *flux, int n, int PM, bool sparse, float2 *vis, int accumulate,
                                      cudaStream_t st);
 
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------

@@ -45,6 +45,11 @@ __host__ __device__ constexpr int tri_row_off(int PM, int n1)
     return o;
 }
 __host__ __device__ constexpr int tri_size(int PM) { return tri_row_off(PM, PM + 1); }
+// One bit per 4-float chunk of the triangle (bit = float offset / 4), set when any of its four
+// coefficients is non-zero, follows the triangle: truncated models skip the
+// load and the FFMAs of empty chunks.  tri_stride = triangle + mask words, padded to 16 bytes.
+__host__ __device__ constexpr int tri_mask_words(int PM) { return (tri_size(PM) / 4 + 31) / 32; }
+__host__ __device__ constexpr int tri_stride(int PM) { return tri_size(PM) + ((tri_mask_words(PM) + 3) & ~3); }
 
 // Per-call channel table, device resident: one block of doubles then floats.
 //   s[f]    = nu_f / c            (FP64, metres -> wavelengths)

@@ -184,6 +184,18 @@ __global__ void pack_coeffs_kernel(const int *__restrict__ coeff_offset, const i
     atomicAdd(&tri[(size_t)lo * tri_floats + tri_index_rt<0>(PM, a, b)], val);
 }
 
+// mask bit c of component k = chunk c (floats 4c..4c+3) of its triangle holds a non-zero coefficient
+__global__ void tri_mask_kernel(float *__restrict__ tri, int n, int tri_floats, int stride)
+{
+    const int chunks = tri_floats / 4;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n * chunks) return;
+    const int k = (int)(i / chunks), c = (int)(i % chunks);
+    const float4 v = *reinterpret_cast<const float4 *>(tri + (size_t)k * stride + 4 * (size_t)c);
+    if (v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f)
+        atomicOr(reinterpret_cast<unsigned int *>(tri + (size_t)k * stride + tri_floats) + c / 32, 1u << (c % 32));
+}
+
 inline int blocks_for(long long n, int t) { return (int)((n + t - 1) / t); }
 
 }  // namespace
@@ -212,18 +224,20 @@ void launch_pack_shapelets(const double *l, const double *m, const double *beta1
                            const double *pa, const double *uv_basis, int n, int PM, GeoS *geo,
                            unsigned int *err, cudaStream_t st)
 {
-    pack_shapelets_kernel<<<blocks_for(n, 128), 128, 0, st>>>(l, m, beta1, beta2, pa, uv_basis, n, tri_size(PM),
+    pack_shapelets_kernel<<<blocks_for(n, 128), 128, 0, st>>>(l, m, beta1, beta2, pa, uv_basis, n, tri_stride(PM),
                                                               geo, err);
 }
 
 void launch_pack_coeffs(const int *coeff_offset, const int *n1, const int *n2, const double *coeff, int n,
                         int n_coeff, int p_max, int PM, float *tri, unsigned int *err, cudaStream_t st)
 {
-    const long long tot = (long long)n * tri_size(PM);
+    const long long tot = (long long)n * tri_stride(PM);
     zero_kernel<<<blocks_for(tot, 256), 256, 0, st>>>(tri, tot);
     if (n_coeff > 0)
         pack_coeffs_kernel<<<blocks_for(n_coeff, 256), 256, 0, st>>>(coeff_offset, n1, n2, coeff, n, n_coeff, p_max,
-                                                                     PM, tri_size(PM), tri, err);
+                                                                     PM, tri_stride(PM), tri, err);
+    tri_mask_kernel<<<blocks_for((long long)n * (tri_size(PM) / 4), 256), 256, 0, st>>>(tri, n, tri_size(PM),
+                                                                                         tri_stride(PM));
 }
 
 }  // namespace woden

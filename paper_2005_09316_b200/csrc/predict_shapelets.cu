@@ -79,16 +79,17 @@ struct HermY {
     }
 };
 
-template <int PM, int NV, int N1>
+template <int PM, int NV, bool SPARSE, int N1>
 struct Rows {
     // process rows N1..PM of the triangle for NV visibilities; gx0[v] = g_{N1}(x_v) * 2^64,
     // gxm[v] = g_{N1-1}(x_v) * 2^64.  One LDS.128 (4 coefficients) feeds 4 NV FFMAs.
     static __device__ __forceinline__ void run(const float *__restrict__ tri, const float (&gy)[NV][PM + 1],
                                                const float (&x)[NV], float (&gx0)[NV], float (&gxm)[NV],
-                                               float (&re)[NV], float (&im)[NV])
+                                               float (&re)[NV], float (&im)[NV], unsigned &mw)
     {
         constexpr int LEN = PM - N1 + 1;
         constexpr int OFF = tri_row_off(PM, N1);
+        (void)mw;
         // NV >= 2 already gives 2 NV independent FFMA chains; NV == 1 splits each into two
         constexpr int NS = NV >= 2 ? 1 : 2;
         float aE[NV][NS], aO[NV][NS];
@@ -99,6 +100,12 @@ struct Rows {
         const float4 *row = reinterpret_cast<const float4 *>(tri + OFF);
 #pragma unroll
         for (int q = 0; q < (LEN + 3) / 4; ++q) {
+            if constexpr (SPARSE) {
+                // truncated model: chunk bit (warp-uniform) says whether any of the 4 coefficients is set
+                const int ch = OFF / 4 + q;
+                if (ch % 32 == 0) mw = reinterpret_cast<const unsigned *>(tri + tri_size(PM))[ch / 32];
+                if (!((mw >> (ch % 32)) & 1u)) continue;
+            }
             const float4 c = row[q];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
@@ -124,7 +131,7 @@ struct Rows {
                 const float g1 = fmaf(cn * x[v], gx0[v], -gxm[v]);
                 gxm[v] = gx0[v]; gx0[v] = g1;
             }
-            Rows<PM, NV, N1 + 1>::run(tri, gy, x, gx0, gxm, re, im);
+            Rows<PM, NV, SPARSE, N1 + 1>::run(tri, gy, x, gx0, gxm, re, im, mw);
         }
     }
 };
@@ -133,10 +140,10 @@ struct Rows {
 // coefficient triangle is broadcast from shared memory; a broadcast LDS.128 occupies the shared
 // memory return path for ~2 cycles per SM (profiles/ncu_r1_*.md), i.e. it can feed at most
 // 2 x 4 warp-FFMAs per NV = 1, half of the FMA pipe's rate: NV = 2 lifts that bound.
-template <int PM, int NV>
+template <int PM, int NV, bool SPARSE>
 __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SParams p)
 {
-    constexpr int TRI = tri_size(PM);
+    constexpr int TRI = tri_stride(PM);             // triangle + chunk mask
     __shared__ __align__(128) float tri_s[TRI];
     __shared__ __align__(8) uint64_t bar;
 
@@ -193,7 +200,8 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
         float xr[NV], xi[NV];
 #pragma unroll
         for (int i = 0; i < NV; ++i) { xr[i] = 0.f; xi[i] = 0.f; }
-        Rows<PM, NV, 0>::run(tri_s, gy, x, gx0, gxm, xr, xi);
+        unsigned mw = 0u;
+        Rows<PM, NV, SPARSE, 0>::run(tri_s, gy, x, gx0, gxm, xr, xi, mw);
         // S7: V += S xi e^{-2 pi i phi}
 #pragma unroll
         for (int i = 0; i < NV; ++i) {
@@ -223,11 +231,12 @@ __global__ void __launch_bounds__(SH_THREADS) predict_shapelets_kernel(const SPa
 constexpr int nv_for(int PM) { return PM <= 16 ? 4 : (PM <= 40 ? 2 : 1); }
 
 template <int PM>
-cudaError_t launch_pm(const SParams &p, int F, cudaStream_t st)
+cudaError_t launch_pm(const SParams &p, int F, bool sparse, cudaStream_t st)
 {
     constexpr int NV = nv_for(PM);
     dim3 grid((unsigned)((p.n_bt + SH_THREADS - 1) / SH_THREADS), (unsigned)((F + NV - 1) / NV));
-    predict_shapelets_kernel<PM, NV><<<grid, SH_THREADS, 0, st>>>(p);
+    if (sparse) predict_shapelets_kernel<PM, NV, true><<<grid, SH_THREADS, 0, st>>>(p);
+    else predict_shapelets_kernel<PM, NV, false><<<grid, SH_THREADS, 0, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -244,7 +253,7 @@ int shapelet_order_bucket(int p_max)
 }
 
 cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
-                                     const float *flux, int n, int PM, float2 *vis, int accumulate,
+                                     const float *flux, int n, int PM, bool sparse, float2 *vis, int accumulate,
                                      cudaStream_t st)
 {
     SParams p;
@@ -253,19 +262,19 @@ cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, con
     p.n_bt = (long long)uvw.T * uvw.B;
     p.B = uvw.B; p.F = uvw.F; p.n = n; p.accumulate = accumulate;
     switch (PM) {
-    case 4: return launch_pm<4>(p, uvw.F, st);
-    case 8: return launch_pm<8>(p, uvw.F, st);
-    case 12: return launch_pm<12>(p, uvw.F, st);
-    case 16: return launch_pm<16>(p, uvw.F, st);
-    case 20: return launch_pm<20>(p, uvw.F, st);
-    case 24: return launch_pm<24>(p, uvw.F, st);
-    case 32: return launch_pm<32>(p, uvw.F, st);
-    case 40: return launch_pm<40>(p, uvw.F, st);
-    case 48: return launch_pm<48>(p, uvw.F, st);
-    case 60: return launch_pm<60>(p, uvw.F, st);
-    case 72: return launch_pm<72>(p, uvw.F, st);
-    case 86: return launch_pm<86>(p, uvw.F, st);
-    case 100: return launch_pm<100>(p, uvw.F, st);
+    case 4: return launch_pm<4>(p, uvw.F, sparse, st);
+    case 8: return launch_pm<8>(p, uvw.F, sparse, st);
+    case 12: return launch_pm<12>(p, uvw.F, sparse, st);
+    case 16: return launch_pm<16>(p, uvw.F, sparse, st);
+    case 20: return launch_pm<20>(p, uvw.F, sparse, st);
+    case 24: return launch_pm<24>(p, uvw.F, sparse, st);
+    case 32: return launch_pm<32>(p, uvw.F, sparse, st);
+    case 40: return launch_pm<40>(p, uvw.F, sparse, st);
+    case 48: return launch_pm<48>(p, uvw.F, sparse, st);
+    case 60: return launch_pm<60>(p, uvw.F, sparse, st);
+    case 72: return launch_pm<72>(p, uvw.F, sparse, st);
+    case 86: return launch_pm<86>(p, uvw.F, sparse, st);
+    case 100: return launch_pm<100>(p, uvw.F, sparse, st);
     }
     return cudaErrorInvalidValue;
 }

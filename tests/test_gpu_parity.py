@@ -236,6 +236,26 @@ def test_shapelets_single_high_order_terms_and_sparse_lists(ctx, torch_mod):
     assert np.abs(V - ref).max() <= TOL * np.abs(cf).sum()
 
 
+@pytest.mark.parametrize("cfg,f_comp", [(5, 0.5), (5, 0.1), (4, 0.3)])
+def test_truncated_shapelet_models_take_the_sparse_kernel(ctx, torch_mod, cfg, f_comp):
+    # PAPER.md section 5.3 (Eq 23-24): basis functions ranked by absolute flux, a fraction kept; the
+    # ragged coefficient lists go through the chunk-skipping kernel variant (PM = 40 NV = 2, PM = 60)
+    from paper_2005_09316_b200 import truncate
+    wl = inputs.make_config(cfg)
+    s = truncate.truncate_shapelets(wl.shapelets, f_comp)
+    assert s.coeff.size < 0.75 * wl.shapelets.coeff.size
+    u, v, w = (a[:2, :1500] for a in (wl.u_m, wl.v_m, wl.w_m))
+    fr = wl.freqs_hz[::48]
+    pmax = int((s.n1 + s.n2).max())
+    V = _run_shapelets(ctx, torch_mod, u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, s.beta1_rad, s.beta2_rad, s.pa_rad,
+                       s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff, pmax)
+    ref = oracle.predict_shapelets(u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, 150e6, s.beta1_rad, s.beta2_rad,
+                                   s.pa_rad, s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff)
+    scale = oracle.tolerance_scale(fr, s.s0_jy, s.alpha, 150e6, s.coeff_offset, s.coeff)
+    assert (np.abs(V - ref) / scale[None, :, None]).max() <= TOL
+    assert np.abs(ref).max() > 1e-3
+
+
 def test_accumulate_zero_components_and_additivity(ctx, torch_mod):
     from paper_2005_09316_b200 import binding
     torch = torch_mod
@@ -290,6 +310,20 @@ def test_simulate_host_matches_device_path(ctx):
     ctx.simulate_host(wl, out)
     dev = _gpu_total(ctx, wl, 0)
     assert np.array_equal(out, dev)
+
+
+def test_simulate_host_time_chunks_are_bit_identical(ctx, torch_mod):
+    # woden_simulate_host predicts in chunks of time steps; 11 steps -> 8 ragged chunks
+    from paper_2005_09316_b200 import binding
+    wl = inputs.make_config(1, n_times=11, n_times_total=11)
+    ctx.set_path(0)
+    out = np.empty((wl.n_times, wl.n_freqs, wl.n_baselines), dtype=np.complex64)
+    ctx.simulate_host(wl, out)
+    dev = _gpu_total(ctx, wl, 0)
+    assert np.array_equal(out, dev)
+    ref = oracle.predict_workload(wl)
+    scale = oracle.workload_tolerance_scale(wl)[None, :, None]
+    assert (np.abs(out - ref) / scale).max() <= TOL
 
 
 def test_error_codes_and_device_side_checks(ctx, torch_mod):
