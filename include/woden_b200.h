@@ -151,6 +151,30 @@ int woden_simulate_host(woden_ctx *ctx,
                         const woden_shapelets_host *shapelets,  /* may be NULL */
                         float *vis_host, void *cuda_stream);
 
+/* The step before the hot path (u,v,w are computed once per time step and only
+ * scaled per channel).  Baseline coordinates in metres from antenna positions by the textbook
+ * rotation (Thompson, Moran & Swenson, cited at PAPER.md:110; reading G14):
+ *   u =  sin H X + cos H Y
+ *   v = -sin d0 cos H X + sin d0 sin H Y + cos d0 Z
+ *   w =  cos d0 cos H X - cos d0 sin H Y + sin d0 Z
+ * with (X,Y,Z) = antenna p - antenna q in the local equatorial frame (X towards the meridian on
+ * the equator, Y east, Z the pole), H the hour angle of the phase centre and d0 its declination.
+ * x_m, y_m, z_m: DEVICE [n_antennas].  hour_angle_rad: HOST [n_times].  u_m, v_m, w_m: DEVICE
+ * [n_times][n_antennas (n_antennas - 1) / 2], pairs p < q in p-major order: exactly what
+ * woden_uvw takes. */
+int woden_uvw_from_antennas(woden_ctx *ctx, int n_antennas,
+                            const double *x_m, const double *y_m, const double *z_m,
+                            int n_times, const double *hour_angle_rad, double dec0_rad,
+                            double *u_m, double *v_m, double *w_m, void *cuda_stream);
+
+/* The time-independent 2x3 matrices M_j of reading G4: rows are the local East
+ * and North unit vectors at direction (l_j, m_j, n_j) in the phase-centre (u,v,w) frame,
+ * e = (p x s)/|p x s|, n = s x e, p = (0, cos d0, sin d0).  l, m: DEVICE [n]; uv_basis: DEVICE
+ * [n][6], the `uv_basis` argument of woden_predict_shapelets.  A component with l^2+m^2 >= 1 or
+ * on the celestial pole gets the identity rows and is counted for woden_check. */
+int woden_shapelet_uv_basis(woden_ctx *ctx, int n, const double *l, const double *m, double dec0_rad,
+                            double *uv_basis, void *cuda_stream);
+
 /* Pipe microbenchmarks used to MEASURE the roofline denominators.
  * Runs `which` (WODEN_PIPE_*) for `iters` dependent-chain-free iterations on every SM and
  * returns warp-instructions per second per GPU in *ops_per_s (thread-ops/s = x32) and the

@@ -35,8 +35,10 @@ def lib():
         L.woden_oracle_hermite_functions.argtypes = [C.c_int, C.c_double, dp]
         L.woden_oracle_hermite_functions.restype = None
         L.woden_oracle_tolerance_scale.argtypes = [C.c_int, dp, C.c_int, dp, dp, C.c_double, ip, dp, dp, C.c_int]
+        L.woden_oracle_uvw.argtypes = [C.c_int, dp, dp, dp, C.c_int, dp, C.c_double, dp, dp, dp]
+        L.woden_oracle_uv_basis.argtypes = [C.c_int, dp, dp, C.c_double, dp]
         for f in (L.woden_oracle_points, L.woden_oracle_gaussians, L.woden_oracle_shapelets,
-                  L.woden_oracle_tolerance_scale):
+                  L.woden_oracle_tolerance_scale, L.woden_oracle_uvw, L.woden_oracle_uv_basis):
             f.restype = C.c_int
         _lib = L
     return _lib
@@ -156,6 +158,24 @@ def tolerance_scale(freqs_hz, s0_jy, alpha, ref_freq_hz, coeff_offset=None, coef
     rc = lib().woden_oracle_tolerance_scale(fr.size, _pd(fr), s0.size, _pd(s0), _pd(al),
                                             float(ref_freq_hz), _pi(off), _pd(cf), _pd(out), int(acc))
     _check(rc, "tolerance_scale")
+    return out
+
+
+def uvw_from_antennas(x_m, y_m, z_m, hour_angle_rad, dec0_rad):
+    """[T, B] u, v, w in metres from local equatorial antenna XYZ (pairs p < q, p-major)."""
+    X, Y, Z, H = _d(x_m), _d(y_m), _d(z_m), _d(hour_angle_rad)
+    n, T = X.size, H.size
+    out = [np.zeros((T, n * (n - 1) // 2), dtype=np.float64) for _ in range(3)]
+    _check(lib().woden_oracle_uvw(n, _pd(X), _pd(Y), _pd(Z), T, _pd(H), float(dec0_rad),
+                                  _pd(out[0]), _pd(out[1]), _pd(out[2])), "uvw")
+    return tuple(out)
+
+
+def shapelet_uv_basis(l, m, dec0_rad) -> np.ndarray:
+    """[n, 6] M_j of reading G4."""
+    l, m = _d(np.atleast_1d(l)), _d(np.atleast_1d(m))
+    out = np.zeros((l.size, 6), dtype=np.float64)
+    _check(lib().woden_oracle_uv_basis(l.size, _pd(l), _pd(m), float(dec0_rad), _pd(out)), "uv_basis")
     return out
 
 

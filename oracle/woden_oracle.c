@@ -241,3 +241,58 @@ int woden_oracle_tolerance_scale(int F, const double *freqs_hz, int n,
     }
     return 0;
 }
+
+/* ---- the step before the hot path -------------------------------------
+ * Baseline (u,v,w) in metres "calculated once per time step" from antenna positions
+ * in the local equatorial frame by the standard interferometry rotation (Thompson, Moran & Swenson,
+ * cited at PAPER.md:110; reading G14), written as the matrix product
+ *   (u,v,w)^T = R(H, d0) (X,Y,Z)^T,   rows of R:  ( sin H,          cos H,         0     )
+ *                                                  (-sin d0 cos H,   sin d0 sin H,  cos d0)
+ *                                                  ( cos d0 cos H,  -cos d0 sin H,  sin d0)
+ * Pairs p < q in p-major order, baseline = antenna p - antenna q.
+ * Pinned by tests/test_oracle_pins.py::test_p16_* (length preservation, R orthonormal, w = projection
+ * on the source direction, special cases). */
+int woden_oracle_uvw(int n_ant, const double *X, const double *Y, const double *Z,
+                     int T, const double *hour_angle, double dec0,
+                     double *u, double *v, double *w)
+{
+    if (n_ant < 2 || T <= 0) return -2;
+    if (!X || !Y || !Z || !hour_angle || !u || !v || !w) return -1;
+    const long long B = (long long)n_ant * (n_ant - 1) / 2;
+    for (int t = 0; t < T; ++t) {
+        const double H = hour_angle[t];
+        const double R[3][3] = {
+            { sin(H),              cos(H),             0.0       },
+            {-sin(dec0) * cos(H),  sin(dec0) * sin(H), cos(dec0) },
+            { cos(dec0) * cos(H), -cos(dec0) * sin(H), sin(dec0) } };
+        long long b = 0;
+        for (int p = 0; p < n_ant; ++p)
+            for (int q = p + 1; q < n_ant; ++q, ++b) {
+                const double d[3] = { X[p] - X[q], Y[p] - Y[q], Z[p] - Z[q] };
+                double o[3];
+                for (int r = 0; r < 3; ++r) o[r] = R[r][0] * d[0] + R[r][1] * d[1] + R[r][2] * d[2];
+                u[(size_t)t * B + b] = o[0]; v[(size_t)t * B + b] = o[1]; w[(size_t)t * B + b] = o[2];
+            }
+    }
+    return 0;
+}
+
+/* M_j of reading G4: local East / North unit vectors at s = (l, m, n) in the
+ * phase-centre (u,v,w) frame; e = (p x s)/|p x s|, north = s x e, p = (0, cos d0, sin d0).
+ * Pinned by test_p14_* (orthonormal, perpendicular to s, identity at the phase centre) and
+ * test_p16_* (equals re-phasing: uvw about the component's own centre = M_j applied to uvw). */
+int woden_oracle_uv_basis(int n, const double *l, const double *m, double dec0, double *M)
+{
+    if (n < 0) return -2;
+    if (n > 0 && (!l || !m || !M)) return -1;
+    const double p[3] = { 0.0, cos(dec0), sin(dec0) };
+    for (int k = 0; k < n; ++k) {
+        const double s[3] = { l[k], m[k], sqrt(1.0 - l[k] * l[k] - m[k] * m[k]) };
+        double e[3] = { p[1] * s[2] - p[2] * s[1], p[2] * s[0] - p[0] * s[2], p[0] * s[1] - p[1] * s[0] };
+        const double en = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+        for (int i = 0; i < 3; ++i) e[i] /= en;
+        const double nn[3] = { s[1] * e[2] - s[2] * e[1], s[2] * e[0] - s[0] * e[2], s[0] * e[1] - s[1] * e[0] };
+        for (int i = 0; i < 3; ++i) { M[6 * (size_t)k + i] = e[i]; M[6 * (size_t)k + 3 + i] = nn[i]; }
+    }
+    return 0;
+}

@@ -31,7 +31,8 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
-           "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate"]
+           "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -94,6 +95,8 @@ def load() -> C.CDLL:
                                       C.POINTER(woden_points_host), C.POINTER(woden_gaussians_host),
                                       C.POINTER(woden_shapelets_host), _vp, _vp]
     L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
+    L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
+    L.woden_shapelet_uv_basis.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, _vp, _vp]
     for name in EXPORTS:
         if name not in ("woden_strerror", "woden_last_error"):
             getattr(L, name).restype = C.c_int
@@ -248,6 +251,28 @@ class Woden:
                                          vis_host.ctypes.data_as(_vp), _stream_handle(stream))
         self._ck(rc, "woden_simulate_host")
         return vis_host
+
+    def uvw_from_antennas(self, x_m, y_m, z_m, hour_angle_rad, dec0_rad, stream=None):
+        """Device [T, B] u, v, w tensors from device antenna XYZ tensors (woden_uvw_from_antennas)."""
+        import torch
+        ha = _hd(hour_angle_rad)
+        n, T = int(x_m.numel()), int(ha.shape[0])
+        out = [torch.empty((T, n * (n - 1) // 2), dtype=torch.float64, device=x_m.device) for _ in range(3)]
+        rc = self._L.woden_uvw_from_antennas(self._ctx, n, _ptr(x_m), _ptr(y_m), _ptr(z_m), T, _hdp(ha),
+                                             float(dec0_rad), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]),
+                                             _stream_handle(stream))
+        self._ck(rc, "woden_uvw_from_antennas")
+        return tuple(out)
+
+    def shapelet_uv_basis(self, l, m, dec0_rad, stream=None):
+        """Device [n, 6] M_j tensor (woden_shapelet_uv_basis)."""
+        import torch
+        n = int(l.numel())
+        out = torch.empty((n, 6), dtype=torch.float64, device=l.device)
+        rc = self._L.woden_shapelet_uv_basis(self._ctx, n, _ptr(l), _ptr(m), float(dec0_rad), _ptr(out),
+                                             _stream_handle(stream))
+        self._ck(rc, "woden_shapelet_uv_basis")
+        return out
 
     def pipe_rate(self, which: str, iters: int = 20000):
         ops, clk = C.c_double(0.0), C.c_double(0.0)

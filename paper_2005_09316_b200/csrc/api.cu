@@ -36,7 +36,7 @@ struct woden_ctx {
     int path = WODEN_PATH_AUTO;
     cudaStream_t last_stream = nullptr;
     std::string last_error;
-    DevBuf geo, flux, tri, chan, err;
+    DevBuf geo, flux, tri, chan, err, hang;
     std::vector<double> chan_freqs;      // frequencies the device channel table was built from
     int chan_F_pad = 0;
     ChanTable ch{};
@@ -197,7 +197,7 @@ int woden_destroy(woden_ctx *ctx)
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
         }
-        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->h_uvw, &ctx->h_comp,
+        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->h_uvw, &ctx->h_comp,
                           &ctx->h_int, &ctx->h_vis})
             b->release();
     }
@@ -493,6 +493,46 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     CU(ctx, cudaStreamSynchronize(st), "simulate sync");
     CU(ctx, cudaStreamSynchronize(ctx->copy_stream), "simulate copy sync");
     ctx->last_stream = st;
+    return WODEN_OK;
+}
+
+int woden_uvw_from_antennas(woden_ctx *ctx, int n_antennas, const double *x_m, const double *y_m, const double *z_m,
+                            int n_times, const double *hour_angle_rad, double dec0_rad, double *u_m, double *v_m,
+                            double *w_m, void *cuda_stream)
+{
+    if (!ctx || !x_m || !y_m || !z_m || !hour_angle_rad || !u_m || !v_m || !w_m) return WODEN_ERR_NULL;
+    if (n_antennas < 2 || n_antennas > 46340 || n_times <= 0 || !std::isfinite(dec0_rad)) return WODEN_ERR_DIM;
+    for (int t = 0; t < n_times; ++t)
+        if (!std::isfinite(hour_angle_rad[t])) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    CU(ctx, ctx->hang.reserve((size_t)n_times * 8), "alloc hour angles");
+    // pageable source: staged by the runtime before the call returns
+    CU(ctx, cudaMemcpyAsync(ctx->hang.p, hour_angle_rad, (size_t)n_times * 8, cudaMemcpyHostToDevice, st),
+       "upload hour angles");
+    CU(ctx, launch_uvw(x_m, y_m, z_m, n_antennas, n_times, static_cast<const double *>(ctx->hang.p), dec0_rad, u_m, v_m,
+                       w_m, st),
+       "uvw launch");
+    return WODEN_OK;
+}
+
+int woden_shapelet_uv_basis(woden_ctx *ctx, int n, const double *l, const double *m, double dec0_rad,
+                            double *uv_basis, void *cuda_stream)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    if (n < 0 || !std::isfinite(dec0_rad)) return WODEN_ERR_DIM;
+    if (n == 0) return WODEN_OK;
+    if (!l || !m || !uv_basis) return WODEN_ERR_NULL;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    int rc = ensure_err(ctx, st);
+    if (rc != WODEN_OK) return rc;
+    CU(ctx, launch_uv_basis(l, m, n, dec0_rad, uv_basis, static_cast<unsigned int *>(ctx->err.p), st),
+       "uv_basis launch");
     return WODEN_OK;
 }
 

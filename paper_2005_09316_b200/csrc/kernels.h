@@ -51,6 +51,12 @@ cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, con
                                      const float *flux, int n, int PM, bool sparse, float2 *vis, int accumulate,
                                      cudaStream_t st);
 
+// ---- geometry before the hot path (geometry.cu) ---------------------
+cudaError_t launch_uvw(const double *X, const double *Y, const double *Z, int n_ant, int T, const double *hour_angle_dev,
+                       double dec0, double *u, double *v, double *w, cudaStream_t st);
+cudaError_t launch_uv_basis(const double *l, const double *m, int n, double dec0, double *M, unsigned int *err,
+                            cudaStream_t st);
+
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
 

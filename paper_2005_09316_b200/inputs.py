@@ -252,6 +252,26 @@ _OBS = {  # config: (array, T, dt_s, F)
 }
 
 
+def make_antennas(config: int, *, t_index0: int = 0, n_times_total: Optional[int] = None,
+                  n_times: Optional[int] = None):
+    """Antenna positions and hour angles behind config 1..5's u_m, v_m, w_m: local equatorial
+    (X, Y, Z) in metres [n_ant], hour angles [T] in radians, and the phase-centre declination --
+    the inputs of woden_uvw_from_antennas.  Same draws as make_config."""
+    if config not in _OBS:
+        raise ValueError(f"config must be 1..5, got {config}")
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + config))
+    arr, T, dt, _ = _OBS[config]
+    if n_times is None:
+        n_times = T
+    if n_times_total is None:
+        n_times_total = max(T, n_times)
+    east, north = _array(rng, arr)
+    lat = np.deg2rad(LATITUDE_DEG)
+    t = np.arange(n_times, dtype=np.float64) + t_index0
+    H = (t - (n_times_total - 1) / 2.0) * dt * 2.0 * np.pi / SIDEREAL_DAY_S
+    return -north * np.sin(lat), east.copy(), north * np.cos(lat), H, np.deg2rad(DEC0_DEG)
+
+
 def make_config_shape(config: int):
     """(array name, T, dt_s, F) of config 1..5 without generating it."""
     if config not in _OBS:

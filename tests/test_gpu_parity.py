@@ -326,6 +326,53 @@ def test_simulate_host_time_chunks_are_bit_identical(ctx, torch_mod):
     assert (np.abs(out - ref) / scale).max() <= TOL
 
 
+def test_uvw_and_uv_basis_on_device_match_the_oracle(ctx, torch_mod):
+    # antenna XYZ -> (u,v,w) once per time step and M_j (G4)
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    X, Y, Z, H, d0 = inputs.make_antennas(5)
+    u, v, w = ctx.uvw_from_antennas(_dev(torch, X), _dev(torch, Y), _dev(torch, Z), H, d0)
+    torch.cuda.synchronize()
+    ru, rv, rw = oracle.uvw_from_antennas(X, Y, Z, H, d0)
+    assert u.shape == (56, 8128)
+    for got, ref in ((u, ru), (v, rv), (w, rw)):
+        assert np.abs(got.cpu().numpy() - ref).max() <= 1e-9          # metres, FP64 both sides
+    wl = inputs.make_config(5)
+    assert np.abs(ru - wl.u_m).max() <= 1e-9 and np.abs(rw - wl.w_m).max() <= 1e-9   # the configs' own uvw
+    for n_ant in (2, 3, 5):                                            # pair indexing at tiny sizes
+        g = ctx.uvw_from_antennas(_dev(torch, X[:n_ant]), _dev(torch, Y[:n_ant]), _dev(torch, Z[:n_ant]), H[:3], d0)
+        r = oracle.uvw_from_antennas(X[:n_ant], Y[:n_ant], Z[:n_ant], H[:3], d0)
+        assert all(np.abs(a.cpu().numpy() - b).max() <= 1e-9 for a, b in zip(g, r))
+    s = wl.shapelets
+    M = ctx.shapelet_uv_basis(_dev(torch, s.l), _dev(torch, s.m), d0)
+    torch.cuda.synchronize(); ctx.check()
+    assert np.abs(M.cpu().numpy() - oracle.shapelet_uv_basis(s.l, s.m, d0)).max() <= 1e-14
+    # end to end: device-made uvw and M_j through the shapelet predictor, against the oracle chain
+    wl1 = inputs.make_config(1)
+    X, Y, Z, H, d0 = inputs.make_antennas(1)
+    u, v, w = ctx.uvw_from_antennas(_dev(torch, X), _dev(torch, Y), _dev(torch, Z), H, d0)
+    s = wl1.shapelets
+    Md = ctx.shapelet_uv_basis(_dev(torch, s.l), _dev(torch, s.m), d0)
+    uvw = binding.Uvw(u, v, w, wl1.freqs_hz)
+    vis = ctx.new_vis(uvw)
+    d = lambda a: _dev(torch, a)
+    di = lambda a: _dev(torch, a, torch.int32)
+    ctx.predict_shapelets(uvw, d(s.l), d(s.m), d(s.s0_jy), d(s.alpha), 150e6, d(s.beta1_rad), d(s.beta2_rad),
+                          d(s.pa_rad), Md, di(s.coeff_offset), len(s.coeff), 5, di(s.n1), di(s.n2), d(s.coeff), vis)
+    torch.cuda.synchronize(); ctx.check()
+    ou, ov, ow = oracle.uvw_from_antennas(X, Y, Z, H, d0)
+    ref = oracle.predict_shapelets(ou, ov, ow, wl1.freqs_hz, s.l, s.m, s.s0_jy, s.alpha, 150e6, s.beta1_rad,
+                                   s.beta2_rad, s.pa_rad, oracle.shapelet_uv_basis(s.l, s.m, d0),
+                                   s.coeff_offset, s.n1, s.n2, s.coeff)
+    scale = oracle.tolerance_scale(wl1.freqs_hz, s.s0_jy, s.alpha, 150e6, s.coeff_offset, s.coeff)
+    assert (np.abs(vis.cpu().numpy() - ref) / scale[None, :, None]).max() <= TOL
+    # a direction outside the unit disk gets identity rows and is counted for woden_check
+    Mb = ctx.shapelet_uv_basis(_dev(torch, [0.9]), _dev(torch, [0.9]), d0)
+    assert np.array_equal(Mb.cpu().numpy(), [[1.0, 0, 0, 0, 1.0, 0]])
+    with pytest.raises(binding.WodenError):
+        ctx.check()
+
+
 def test_error_codes_and_device_side_checks(ctx, torch_mod):
     from paper_2005_09316_b200 import binding
     torch = torch_mod

@@ -411,3 +411,59 @@ def test_tolerance_scale_definition():
     ref += (np.abs(wl.gaussians.s0_jy) * fr ** wl.gaussians.alpha).sum(1)
     ref += (np.abs(wl.shapelets.s0_jy) * fr ** wl.shapelets.alpha).sum(1) * np.abs(wl.shapelets.coeff).sum()
     assert np.allclose(sc, ref, rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- P16 (NEXT-2)
+def test_p16_uvw_rotation_special_cases_lengths_and_projection():
+    rng = np.random.default_rng(16)
+    n = 7
+    X, Y, Z = rng.normal(0, 800.0, (3, n))
+    # explicit pair order for 3 antennas: (0,1), (0,2), (1,2); baseline = antenna p - antenna q
+    u, v, w = oracle.uvw_from_antennas(X[:3], Y[:3], Z[:3], [0.0], 0.0)
+    assert np.allclose(u[0], [Y[0] - Y[1], Y[0] - Y[2], Y[1] - Y[2]], atol=1e-12)      # H = 0, d0 = 0: u = Y
+    assert np.allclose(v[0], [Z[0] - Z[1], Z[0] - Z[2], Z[1] - Z[2]], atol=1e-12)      #                v = Z
+    assert np.allclose(w[0], [X[0] - X[1], X[0] - X[2], X[1] - X[2]], atol=1e-12)      #                w = X
+    u, v, w = oracle.uvw_from_antennas(X[:2], Y[:2], Z[:2], [0.0, np.pi / 2], np.pi / 2)
+    assert np.allclose([u[0, 0], v[0, 0], w[0, 0]], [Y[0] - Y[1], -(X[0] - X[1]), Z[0] - Z[1]], atol=1e-12)   # pole
+    u, v, w = oracle.uvw_from_antennas(X[:2], Y[:2], Z[:2], [np.pi / 2], 0.0)
+    assert np.allclose([u[0, 0], v[0, 0], w[0, 0]], [X[0] - X[1], Z[0] - Z[1], -(Y[0] - Y[1])], atol=1e-12)
+    # general case: a rotation preserves length; w is the projection on the source direction
+    H = np.array([-0.7, 0.0, 0.3, 2.9]); d0 = np.deg2rad(-37.0)
+    u, v, w = oracle.uvw_from_antennas(X, Y, Z, H, d0)
+    p, q = inputs.baseline_pairs(n)
+    bx, by, bz = X[p] - X[q], Y[p] - Y[q], Z[p] - Z[q]
+    assert np.allclose(u * u + v * v + w * w, (bx * bx + by * by + bz * bz)[None, :], rtol=1e-13)
+    for t, h in enumerate(H):
+        s0 = np.array([np.cos(d0) * np.cos(h), -np.cos(d0) * np.sin(h), np.sin(d0)])     # source direction in XYZ
+        assert np.allclose(w[t], bx * s0[0] + by * s0[1] + bz * s0[2], atol=1e-10)
+        east = np.array([np.sin(h), np.cos(h), 0.0])                                      # d s0 / dH direction
+        assert np.allclose(u[t], bx * east[0] + by * east[1], atol=1e-10)
+
+
+def test_p16_uv_basis_is_rephasing_to_the_component_centre():
+    # the shapelet's u,v are "calculated with a phase-centre ... which corresponds to
+    # the central position" of the shapelet.  Reading G4 replaces that by the time-independent M_j;
+    # here the two are shown equal using the oracle's own uvw routine at the component's (H_j, d_j).
+    rng = np.random.default_rng(61)
+    X, Y, Z = rng.normal(0, 900.0, (3, 6))
+    d0 = np.deg2rad(-37.0)
+    l = np.array([0.0, 0.12, -0.3, 0.02]); m = np.array([0.0, -0.2, 0.25, 0.4])
+    M = oracle.shapelet_uv_basis(l, m, d0).reshape(-1, 2, 3)
+    assert np.allclose(M[0], [[1, 0, 0], [0, 1, 0]], atol=1e-15)            # identity at the phase centre
+    sv = np.stack([l, m, np.sqrt(1 - l * l - m * m)], axis=1)
+    for j in range(len(l)):
+        assert np.allclose(M[j] @ M[j].T, np.eye(2), atol=1e-15)            # orthonormal rows
+        assert np.allclose(M[j] @ sv[j], 0.0, atol=1e-15)                   # perpendicular to s
+    for H0 in (-1.1, 0.0, 0.4):
+        u0, v0, w0 = oracle.uvw_from_antennas(X, Y, Z, [H0], d0)
+        R0 = np.array([[np.sin(H0), np.cos(H0), 0.0],
+                       [-np.sin(d0) * np.cos(H0), np.sin(d0) * np.sin(H0), np.cos(d0)],
+                       [np.cos(d0) * np.cos(H0), -np.cos(d0) * np.sin(H0), np.sin(d0)]])
+        for j in range(len(l)):
+            sx = R0.T @ sv[j]                                                # component direction in XYZ
+            dj, Hj = np.arcsin(sx[2]), np.arctan2(-sx[1], sx[0])
+            uj, vj, _ = oracle.uvw_from_antennas(X, Y, Z, [Hj], dj)
+            got = M[j] @ np.stack([u0[0], v0[0], w0[0]])
+            assert np.allclose(got[0], uj[0], atol=1e-9) and np.allclose(got[1], vj[0], atol=1e-9)
+    # the generator's matrices (used for configs 1, 4, 5) are the same ones
+    assert np.allclose(inputs.local_uv_basis(l, m, d0), oracle.shapelet_uv_basis(l, m, d0), atol=1e-15)
