@@ -175,6 +175,26 @@ int woden_uvw_from_antennas(woden_ctx *ctx, int n_antennas,
 int woden_shapelet_uv_basis(woden_ctx *ctx, int n, const double *l, const double *m, double dec0_rad,
                             double *uv_basis, void *cuda_stream);
 
+/* The consumer of the predicted visibilities in the paper (section 5.1, Eq 18-22): one
+ * complex gain per antenna, fitted independently for every (time, frequency) cell by n_iter
+ * (the paper: 10) passes of  x = [A^T A]^-1 A^T b  on the linearised residual
+ *   R_ij = V_ij - g_i g_j^* I_ij ~ e_i g_j^* I_ij + g_i e_j^* I_ij,   g <- g + e,  from g = 1
+ * (readings G15, G16: Eq 18's g_i g_i^* is read g_i g_j^*; the overall phase is unconstrained, so
+ * each step is the minimum-norm least-squares solution).  vis_data (V) and vis_model (I): DEVICE
+ * complex64 [n_cells][n_antennas (n_antennas - 1) / 2], i.e. a woden_predict_* buffer viewed as
+ * n_cells = n_times * n_freqs cells of all pairs i < j in i-major order.  gains: DEVICE complex128
+ * [n_cells][n_antennas], written.  n_antennas is limited by shared memory (<= 164).
+ * The spline smoothing of the gains across the band (:237) is not implemented. */
+int woden_calibrate_gains(woden_ctx *ctx, int n_antennas, long long n_cells,
+                          const float *vis_data, const float *vis_model, int n_iter,
+                          double *gains, void *cuda_stream);
+
+/* vis_out = V_ij - g_i g_j^* I_ij (Eq 20 with the fitted gains), same layouts; vis_out may alias
+ * vis_data. */
+int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells,
+               const float *vis_data, const float *vis_model, const double *gains,
+               float *vis_out, void *cuda_stream);
+
 /* Pipe microbenchmarks used to MEASURE the roofline denominators.
  * Runs `which` (WODEN_PIPE_*) for `iters` dependent-chain-free iterations on every SM and
  * returns warp-instructions per second per GPU in *ops_per_s (thread-ops/s = x32) and the

@@ -32,7 +32,7 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -97,6 +97,8 @@ def load() -> C.CDLL:
     L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
     L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
     L.woden_shapelet_uv_basis.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, _vp, _vp]
+    L.woden_calibrate_gains.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, C.c_int, _vp, _vp]
+    L.woden_peel.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     for name in EXPORTS:
         if name not in ("woden_strerror", "woden_last_error"):
             getattr(L, name).restype = C.c_int
@@ -272,6 +274,31 @@ class Woden:
         rc = self._L.woden_shapelet_uv_basis(self._ctx, n, _ptr(l), _ptr(m), float(dec0_rad), _ptr(out),
                                              _stream_handle(stream))
         self._ck(rc, "woden_shapelet_uv_basis")
+        return out
+
+    def calibrate_gains(self, n_antennas: int, vis_data, vis_model, n_iter: int = 10, stream=None):
+        """complex128 gains [..., n_antennas] for complex64 [..., B] device tensors (woden_calibrate_gains)."""
+        import torch
+        nb = n_antennas * (n_antennas - 1) // 2
+        if vis_data.shape != vis_model.shape or vis_data.shape[-1] != nb or vis_data.dtype != torch.complex64:
+            raise ValueError("vis_data / vis_model must be complex64 [..., n_ant (n_ant - 1) / 2]")
+        cells = vis_data.numel() // nb
+        gains = torch.empty(tuple(vis_data.shape[:-1]) + (n_antennas,), dtype=torch.complex128, device=vis_data.device)
+        rc = self._L.woden_calibrate_gains(self._ctx, int(n_antennas), cells, _ptr(vis_data), _ptr(vis_model),
+                                           int(n_iter), _ptr(gains), _stream_handle(stream))
+        self._ck(rc, "woden_calibrate_gains")
+        return gains
+
+    def peel(self, n_antennas: int, vis_data, vis_model, gains, out=None, stream=None):
+        """V - g_i g_j^* I (woden_peel)."""
+        import torch
+        nb = n_antennas * (n_antennas - 1) // 2
+        cells = vis_data.numel() // nb
+        if out is None:
+            out = torch.empty_like(vis_data)
+        rc = self._L.woden_peel(self._ctx, int(n_antennas), cells, _ptr(vis_data), _ptr(vis_model), _ptr(gains),
+                                _ptr(out), _stream_handle(stream))
+        self._ck(rc, "woden_peel")
         return out
 
     def pipe_rate(self, which: str, iters: int = 20000):

@@ -536,6 +536,38 @@ int woden_shapelet_uv_basis(woden_ctx *ctx, int n, const double *l, const double
     return WODEN_OK;
 }
 
+int woden_calibrate_gains(woden_ctx *ctx, int n_antennas, long long n_cells, const float *vis_data,
+                          const float *vis_model, int n_iter, double *gains, void *cuda_stream)
+{
+    if (!ctx || !vis_data || !vis_model || !gains) return WODEN_ERR_NULL;
+    if (n_antennas < 2 || n_cells <= 0 || n_cells > 2147483647LL || n_iter < 0) return WODEN_ERR_DIM;
+    if (calibrate_smem_bytes(n_antennas) > 227u * 1024u) return WODEN_ERR_DIM;     // W must fit shared memory
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    CU(ctx, launch_calibrate(reinterpret_cast<const float2 *>(vis_data), reinterpret_cast<const float2 *>(vis_model),
+                             reinterpret_cast<double2 *>(gains), n_antennas, n_cells, n_iter, st),
+       "calibrate launch");
+    return WODEN_OK;
+}
+
+int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells, const float *vis_data, const float *vis_model,
+               const double *gains, float *vis_out, void *cuda_stream)
+{
+    if (!ctx || !vis_data || !vis_model || !gains || !vis_out) return WODEN_ERR_NULL;
+    if (n_antennas < 2 || n_antennas > 46340 || n_cells <= 0) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    CU(ctx, launch_peel(reinterpret_cast<const float2 *>(vis_data), reinterpret_cast<const float2 *>(vis_model),
+                        reinterpret_cast<const double2 *>(gains), reinterpret_cast<float2 *>(vis_out), n_antennas,
+                        n_cells, st),
+       "peel launch");
+    return WODEN_OK;
+}
+
 int woden_pipe_rate(woden_ctx *ctx, int which, int iters, double *thread_ops_per_s, double *sm_clock_hz)
 {
     if (!ctx || !thread_ops_per_s || !sm_clock_hz) return WODEN_ERR_NULL;

@@ -57,6 +57,13 @@ cudaError_t launch_uvw(const double *X, const double *Y, const double *Z, int n_
 cudaError_t launch_uv_basis(const double *l, const double *m, int n, double dec0, double *M, unsigned int *err,
                             cudaStream_t st);
 
+// ---- gain calibration and peel (calibrate.cu) -------------------------
+size_t calibrate_smem_bytes(int N);
+cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *gains, int N, long long cells,
+                             int n_iter, cudaStream_t st);
+cudaError_t launch_peel(const float2 *data, const float2 *model, const double2 *gains, float2 *out, int N,
+                        long long cells, cudaStream_t st);
+
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
 
