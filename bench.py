@@ -425,6 +425,62 @@ def run_truncation(args):
     return 0
 
 
+def run_peel(args):
+    """The paper's consumer of the predicted visibilities (section 5.1): fit one complex gain
+    per antenna and (time, frequency) cell by 10 passes of Eq 22, then subtract the calibrated model.
+    "Observed" = config 5's sky through the predictors, model = its truncated version (Eq 23-24,
+    f_comp = 0.8) through the predictors."""
+    import torch
+    from paper_2005_09316_b200 import binding, truncate
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --peel: no CUDA device")
+    wl = inputs.make_config(args.config)
+    n_ant = int(round((1 + (1 + 8 * wl.n_baselines) ** 0.5) / 2))
+    ctx = binding.Woden(0)
+    dw = binding.DeviceWorkload(wl)
+    full = dw.predict(ctx)
+    wl_t = inputs.make_config(args.config)
+    wl_t.points = truncate.truncate_components(wl.points, 0.8)
+    wl_t.gaussians = truncate.truncate_components(wl.gaussians, 0.8)
+    wl_t.shapelets = truncate.truncate_shapelets(wl.shapelets, 0.8)
+    model = binding.DeviceWorkload(wl_t).predict(ctx)
+    out = torch.empty_like(full)
+    torch.cuda.synchronize()
+
+    def timed(fn, reps):
+        fn(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+
+    g = [None]
+    ms_cal = timed(lambda: g.__setitem__(0, ctx.calibrate_gains(n_ant, full, model, 10)), max(3, args.steps))
+    ms_peel = timed(lambda: ctx.peel(n_ant, full, model, g[0], out=out), max(3, args.steps))
+    ctx.check()
+    cells = wl.n_times * wl.n_freqs
+    before = float(torch.sum(torch.abs(full - model) ** 2).item())
+    after = float(torch.sum(torch.abs(out) ** 2).item())
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    gbs = 3 * full.numel() * 8 / (ms_peel * 1e-3) / 1e9
+    print(json.dumps({
+        "peel": {"workload": f"config {wl.config}: {cells} cells x {n_ant} antennas ({wl.n_baselines} baselines)",
+                 "calibrate_ms": ms_cal, "cell_fits_per_s": cells / (ms_cal * 1e-3), "iterations": 10,
+                 "peel_ms": ms_peel,
+                 "peel_roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+                                   "peak_source": "measured" if peaks else "fallback",
+                                   "algorithmic_bytes_per_visibility": 24},
+                 "residual_power_raw_model": before, "residual_power_after_peel": after}}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -435,6 +491,8 @@ def main():
     ap.add_argument("--path", choices=["auto", "general"], default="auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipes", action="store_true", help="print the measured pipe rates and exit")
+    ap.add_argument("--peel", action="store_true",
+                    help="time the gain fit and peel of PAPER.md section 5.1 on the config and exit")
     ap.add_argument("--truncation", action="store_true",
                     help="GPU time vs kept fraction of components (PAPER.md section 5.3) and exit")
     args = ap.parse_args()
@@ -442,6 +500,8 @@ def main():
         return run_pipes(args)
     if args.truncation:
         return run_truncation(args)
+    if args.peel:
+        return run_peel(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -556,7 +556,7 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells, const float *v
                const double *gains, float *vis_out, void *cuda_stream)
 {
     if (!ctx || !vis_data || !vis_model || !gains || !vis_out) return WODEN_ERR_NULL;
-    if (n_antennas < 2 || n_antennas > 46340 || n_cells <= 0) return WODEN_ERR_DIM;
+    if (n_antennas < 2 || n_antennas > 3000 || n_cells <= 0 || n_cells > 2147483647LL) return WODEN_ERR_DIM;
     Bind bind(ctx);
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

@@ -23,7 +23,7 @@
 namespace woden {
 namespace {
 
-constexpr int CAL_THREADS = 256;
+constexpr int CAL_THREADS = 512;
 
 struct CalParams {
     const float2 *data, *model;   // [cells][B] complex64
@@ -31,6 +31,7 @@ struct CalParams {
     int N, n_iter, cg_max;
     long long B;
     double cg_tol2;               // squared relative residual at which CG stops
+    double cg_abs2;               // squared absolute size of the remaining correction at which CG stops
 };
 
 // index of pair (i, j), i < j, in i-major order
@@ -81,6 +82,11 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
     double *p0 = r1 + N, *p1 = p0 + N;           // CG directions (pre-multiplied by q for the product)
     double *a0 = p1 + N, *a1 = a0 + N;           // M p
     double *scratch = a1 + N;                    // [4][CAL_THREADS / 32]
+    double *part = scratch + 4 * (CAL_THREADS / 32);   // [split][2][N] partial products, split N <= CAL_THREADS
+    double *invd = part + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS);    // Jacobi preconditioner 1 / (q d)
+    double2 *qp = reinterpret_cast<double2 *>(invd + N);   // q o (p0, p1); offset N (N + 15) + 4 (CAL_THREADS / 32) + 2 max(N, CAL_THREADS) doubles is even: 16-byte aligned
+    const int split = N >= CAL_THREADS ? 1 : CAL_THREADS / N;
+    const int jchunk = (N + split - 1) / split;
 
     const float2 *V = p.data + (size_t)blockIdx.x * p.B;
     const float2 *I = p.model + (size_t)blockIdx.x * p.B;
@@ -101,12 +107,13 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
     for (int it = 0; it < p.n_iter; ++it) {
         for (int i = tid; i < N; i += CAL_THREADS) q[i] = gre[i] * gre[i] + gim[i] * gim[i];
         __syncthreads();
-        // d_i and rho_i: thread i gathers over all partners j
-        for (int i = tid; i < N; i += CAL_THREADS) {
+        // d_i and rho_i: one warp per antenna i, lanes over the partners j (coalesced rows of I, V)
+        for (int i = tid >> 5; i < N; i += CAL_THREADS / 32) {
             double di = 0.0, sr = 0.0, si = 0.0;
-            for (int j = 0; j < N; ++j) {
+#pragma unroll 4
+            for (int j = tid & 31; j < N; j += 32) {
                 if (j == i) continue;
-                di = fma(W[(size_t)j * N + i], q[j], di);
+                di = fma(W[(size_t)i * N + j], q[j], di);
                 const long long b = i < j ? pair_index(i, j, N) : pair_index(j, i, N);
                 const float2 m = I[b], v = V[b];
                 // C_ij = conj(I_ij) V_ij for the ordered pair (i, j); the stored pair is (min, max)
@@ -116,11 +123,14 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
                 sr += gre[j] * cr - gim[j] * ci;             // g_j C_ij
                 si += gre[j] * ci + gim[j] * cr;
             }
-            d[i] = di;
-            const double rr = sr - gre[i] * di, ri = si - gim[i] * di;       // r_i = sum - g_i d_i
-            // rho = r / g, then scaled by q = |g|^2:  q rho = r conj(g)
-            rhs0[i] = rr * gre[i] + ri * gim[i];
-            rhs1[i] = ri * gre[i] - rr * gim[i];
+            di = warp_sum(di); sr = warp_sum(sr); si = warp_sum(si);
+            if ((tid & 31) == 0) {
+                d[i] = di;
+                const double rr = sr - gre[i] * di, ri = si - gim[i] * di;       // r_i = sum - g_i d_i
+                // rho = r / g, then scaled by q = |g|^2:  q rho = r conj(g)
+                rhs0[i] = rr * gre[i] + ri * gim[i];
+                rhs1[i] = ri * gre[i] - rr * gim[i];
+            }
         }
         __syncthreads();
         // range projection of the singular system's right-hand side (null vector: all ones)
@@ -131,29 +141,51 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
             const double mean = s[0] / N;
             for (int i = tid; i < N; i += CAL_THREADS) rhs1[i] -= mean;
         }
-        // Jacobi-preconditioned CG on both systems, x = 0 start
-        double rz[2] = {0.0, 0.0};
+        // Jacobi-preconditioned CG on both systems, x = 0 start.  qp[j] = q_j (p0_j, p1_j) is formed
+        // once per iteration so the product loop reads one W word and one 16-byte broadcast per j.
+        double rz[3] = {0.0, 0.0, 0.0};
         for (int i = tid; i < N; i += CAL_THREADS) {
             const double dg = q[i] * d[i], inv = dg > 0.0 ? 1.0 / dg : 0.0;
+            invd[i] = inv;
+            rz[2] += dg;
             x0[i] = 0.0; x1[i] = 0.0;
             r0[i] = rhs0[i]; r1[i] = rhs1[i];
             p0[i] = r0[i] * inv; p1[i] = r1[i] * inv;
+            qp[i] = make_double2(q[i] * p0[i], q[i] * p1[i]);
             rz[0] += r0[i] * p0[i]; rz[1] += r1[i] * p1[i];
         }
-        block_sum<2>(rz, scratch);
-        const double rz_first0 = rz[0], rz_first1 = rz[1];
+        block_sum<3>(rz, scratch);
+        // stop at a residual reduced by sqrt(cg_tol2), or once the correction it stands for is below
+        // cg_abs in the (q d)-weighted rms of eps (late outer iterations start almost converged)
+        const double floor0 = fmax(p.cg_tol2 * rz[0], p.cg_abs2 * rz[2]);
+        const double floor1 = fmax(p.cg_tol2 * rz[1], p.cg_abs2 * rz[2]);
         for (int cg = 0; cg < p.cg_max; ++cg) {
-            const bool live0 = rz[0] > p.cg_tol2 * rz_first0 && rz[0] > 0.0;
-            const bool live1 = rz[1] > p.cg_tol2 * rz_first1 && rz[1] > 0.0;
+            const bool live0 = rz[0] > floor0;
+            const bool live1 = rz[1] > floor1;
             if (!live0 && !live1) break;
+            // t = W (q o p): `split` thread groups each take a slice of the partners j of antenna i
+            if (tid < split * N) {
+                const int i = tid % N, h = tid / N;
+                const int j0 = h * jchunk, j1 = min(N, j0 + jchunk);
+                const double *Wc = W + i;
+                double t0 = 0.0, t1 = 0.0, u0 = 0.0, u1 = 0.0;
+                int j = j0;
+#pragma unroll 4
+                for (; j + 1 < j1; j += 2) {
+                    const double wa = Wc[(size_t)j * N], wb = Wc[(size_t)(j + 1) * N];
+                    const double2 a = qp[j], b = qp[j + 1];
+                    t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1);
+                    u0 = fma(wb, b.x, u0); u1 = fma(wb, b.y, u1);
+                }
+                if (j < j1) { const double wa = Wc[(size_t)j * N]; const double2 a = qp[j]; t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1); }
+                part[(2 * h) * N + i] = t0 + u0;
+                part[(2 * h + 1) * N + i] = t1 + u1;
+            }
+            __syncthreads();
             double pa[2] = {0.0, 0.0};
             for (int i = tid; i < N; i += CAL_THREADS) {
                 double t0 = 0.0, t1 = 0.0;
-                for (int j = 0; j < N; ++j) {
-                    const double wq = W[(size_t)j * N + i] * q[j];
-                    t0 = fma(wq, p0[j], t0);
-                    t1 = fma(wq, p1[j], t1);
-                }
+                for (int h = 0; h < split; ++h) { t0 += part[(2 * h) * N + i]; t1 += part[(2 * h + 1) * N + i]; }
                 a0[i] = q[i] * (d[i] * p0[i] + t0);
                 a1[i] = q[i] * (d[i] * p1[i] - t1);
                 pa[0] += p0[i] * a0[i]; pa[1] += p1[i] * a1[i];
@@ -163,18 +195,17 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
             const double al1 = live1 && pa[1] > 0.0 ? rz[1] / pa[1] : 0.0;
             double rzn[2] = {0.0, 0.0};
             for (int i = tid; i < N; i += CAL_THREADS) {
-                const double dg = q[i] * d[i], inv = dg > 0.0 ? 1.0 / dg : 0.0;
                 x0[i] += al0 * p0[i]; x1[i] += al1 * p1[i];
                 r0[i] -= al0 * a0[i]; r1[i] -= al1 * a1[i];
-                rzn[0] += r0[i] * r0[i] * inv; rzn[1] += r1[i] * r1[i] * inv;
+                rzn[0] += r0[i] * r0[i] * invd[i]; rzn[1] += r1[i] * r1[i] * invd[i];
             }
             block_sum<2>(rzn, scratch);
-            const double be0 = live0 && rz[0] > 0.0 ? rzn[0] / rz[0] : 0.0;
-            const double be1 = live1 && rz[1] > 0.0 ? rzn[1] / rz[1] : 0.0;
+            const double be0 = live0 ? rzn[0] / rz[0] : 0.0;
+            const double be1 = live1 ? rzn[1] / rz[1] : 0.0;
             for (int i = tid; i < N; i += CAL_THREADS) {
-                const double dg = q[i] * d[i], inv = dg > 0.0 ? 1.0 / dg : 0.0;
-                if (live0) p0[i] = r0[i] * inv + be0 * p0[i];
-                if (live1) p1[i] = r1[i] * inv + be1 * p1[i];
+                if (live0) p0[i] = r0[i] * invd[i] + be0 * p0[i];
+                if (live1) p1[i] = r1[i] * invd[i] + be1 * p1[i];
+                qp[i] = make_double2(live0 ? q[i] * p0[i] : 0.0, live1 ? q[i] * p1[i] : 0.0);
             }
             if (live0) rz[0] = rzn[0];
             if (live1) rz[1] = rzn[1];
@@ -200,30 +231,40 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
         p.gains[(size_t)blockIdx.x * N + i] = make_double2(gre[i], gim[i]);
 }
 
-// out = V - g_i g_j^* I (Eq 20 with the fitted gains), one thread per visibility
-__global__ void peel_kernel(const float2 *__restrict__ data, const float2 *__restrict__ model,
-                            const double2 *__restrict__ gains, float2 *__restrict__ out, int N, long long B,
-                            long long total)
+// out = V - g_i g_j^* I (Eq 20 with the fitted gains).  One CTA per cell: gains in shared memory,
+// one warp per baseline row i, lanes over j > i (consecutive visibilities).  HBM-bound: 24 B per
+// visibility.
+__global__ void __launch_bounds__(CAL_THREADS) peel_kernel(const float2 *__restrict__ data,
+                                                           const float2 *__restrict__ model,
+                                                           const double2 *__restrict__ gains, float2 *__restrict__ out,
+                                                           int N, long long B)
 {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= total) return;
-    const long long cell = idx / B, b = idx - cell * B;
-    const double nn = 2.0 * N - 1.0;
-    int i = (int)floor((nn - sqrt(nn * nn - 8.0 * (double)b)) * 0.5);
-    if (i < 0) i = 0;
-    if (i > N - 2) i = N - 2;
-    while (i > 0 && (long long)i * (2LL * N - i - 1) / 2 > b) --i;
-    while ((long long)(i + 1) * (2LL * N - i - 2) / 2 <= b) ++i;
-    const int j = (int)(b - (long long)i * (2LL * N - i - 1) / 2) + i + 1;
-    const double2 gi = gains[cell * N + i], gj = gains[cell * N + j];
-    const double pr = gi.x * gj.x + gi.y * gj.y, pi = gi.y * gj.x - gi.x * gj.y;      // g_i conj(g_j)
-    const float2 m = model[idx], v = data[idx];
-    out[idx] = make_float2((float)((double)v.x - (pr * m.x - pi * m.y)), (float)((double)v.y - (pr * m.y + pi * m.x)));
+    extern __shared__ __align__(16) double2 gs[];
+    const size_t cell = blockIdx.x;
+    for (int i = threadIdx.x; i < N; i += CAL_THREADS) gs[i] = gains[cell * N + i];
+    __syncthreads();
+    const float2 *v = data + cell * B, *m = model + cell * B;
+    float2 *o = out + cell * B;
+    for (int i = threadIdx.x >> 5; i < N - 1; i += CAL_THREADS / 32) {
+        const double2 gi = gs[i];
+        const long long row = pair_index(i, i + 1, N);
+        for (int j = i + 1 + (threadIdx.x & 31); j < N; j += 32) {
+            const double2 gj = gs[j];
+            const double pr = gi.x * gj.x + gi.y * gj.y, pi = gi.y * gj.x - gi.x * gj.y;      // g_i conj(g_j)
+            const long long b = row + (j - i - 1);
+            const float2 mm = m[b], vv = v[b];
+            o[b] = make_float2((float)((double)vv.x - (pr * mm.x - pi * mm.y)),
+                               (float)((double)vv.y - (pr * mm.y + pi * mm.x)));
+        }
+    }
 }
 
 }  // namespace
 
-size_t calibrate_smem_bytes(int N) { return ((size_t)N * N + 16 * (size_t)N + 4 * (CAL_THREADS / 32)) * sizeof(double); }
+size_t calibrate_smem_bytes(int N)
+{
+    return ((size_t)N * N + 20 * (size_t)N + 2 + 4 * (CAL_THREADS / 32) + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS)) * sizeof(double);
+}
 
 cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *gains, int N, long long cells, int n_iter,
                              cudaStream_t st)
@@ -233,6 +274,7 @@ cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *g
     p.B = (long long)N * (N - 1) / 2;
     p.cg_max = 2 * N + 10;
     p.cg_tol2 = 1e-26;             // residual reduced by 1e-13
+    p.cg_abs2 = 1e-28;             // or the remaining relative gain correction below 1e-14
     const size_t smem = calibrate_smem_bytes(N);
     cudaError_t e = cudaFuncSetAttribute(calibrate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -243,8 +285,8 @@ cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *g
 cudaError_t launch_peel(const float2 *data, const float2 *model, const double2 *gains, float2 *out, int N,
                         long long cells, cudaStream_t st)
 {
-    const long long B = (long long)N * (N - 1) / 2, total = cells * B;
-    peel_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(data, model, gains, out, N, B, total);
+    const long long B = (long long)N * (N - 1) / 2;
+    peel_kernel<<<(unsigned)cells, CAL_THREADS, (size_t)N * sizeof(double2), st>>>(data, model, gains, out, N, B);
     return cudaGetLastError();
 }
 
