@@ -179,7 +179,7 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
 
         Seed<GAUSS> sd;
         make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, ds, sd);
-#pragma unroll 1
+#pragma unroll (GAUSS ? 2 : 1)
         for (int k = 0; k < KB; ++k) {
             // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
             Seed<GAUSS> nx;
