@@ -77,6 +77,17 @@ int woden_check(woden_ctx *ctx);
 #define WODEN_PATH_GENERAL 1
 int woden_set_path(woden_ctx *ctx, int path);
 
+/* Shapelet engine selection (measurement / testing).  Default WODEN_SHAPELET_AUTO.
+ *   REGISTER : FP32 register path, one FFMA per coefficient (predict_shapelets.cu)
+ *   TENSOR   : the coefficient sum of each shapelet as a batched matrix product on the tensor cores
+ *              (tcgen05, FP16 hi + lo operands, FP32 accumulation in TMEM; predict_shapelets_mma.cu)
+ *   AUTO     : whichever measured faster for the order
+ * All meet the same parity tolerance. */
+#define WODEN_SHAPELET_AUTO     0
+#define WODEN_SHAPELET_REGISTER 1
+#define WODEN_SHAPELET_TENSOR   2
+int woden_set_shapelet_path(woden_ctx *ctx, int path);
+
 /* Baseline coordinates and channels ("array layout and observation parameters"). */
 typedef struct {
     int n_baselines, n_times, n_freqs;

@@ -26,13 +26,16 @@ WODEN_ERR_DATA = -6
 WODEN_MAX_ORDER = 100
 WODEN_PATH_AUTO = 0
 WODEN_PATH_GENERAL = 1
+WODEN_SHAPELET_AUTO = 0
+WODEN_SHAPELET_REGISTER = 1
+WODEN_SHAPELET_TENSOR = 2
 PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA_IMM": 6, "F2F": 7,
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -86,6 +89,7 @@ def load() -> C.CDLL:
     L.woden_last_error.restype = C.c_char_p
     L.woden_check.argtypes = [_vp]
     L.woden_set_path.argtypes = [_vp, C.c_int]
+    L.woden_set_shapelet_path.argtypes = [_vp, C.c_int]
     common = [_vp, C.POINTER(woden_uvw), C.c_int, _vp, _vp, _vp, _vp, C.c_double]
     tail = [_vp, C.c_int, _vp]
     L.woden_predict_points.argtypes = common + tail
@@ -184,6 +188,9 @@ class Woden:
 
     def set_path(self, path: int):
         self._ck(self._L.woden_set_path(self._ctx, int(path)), "woden_set_path")
+
+    def set_shapelet_path(self, path: int):
+        self._ck(self._L.woden_set_shapelet_path(self._ctx, int(path)), "woden_set_shapelet_path")
 
     def check(self):
         self._ck(self._L.woden_check(self._ctx), "woden_check")

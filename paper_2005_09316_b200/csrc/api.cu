@@ -7,6 +7,8 @@
 #include <string>
 #include <vector>
 
+#include <cuda_fp16.h>
+
 #include "../../include/woden_b200.h"
 #include "kernels.h"
 
@@ -36,7 +38,8 @@ struct woden_ctx {
     int path = WODEN_PATH_AUTO;
     cudaStream_t last_stream = nullptr;
     std::string last_error;
-    DevBuf geo, flux, tri, chan, err, hang;
+    DevBuf geo, flux, tri, chan, err, hang, bmat, bscale;
+    int shapelet_path = WODEN_SHAPELET_AUTO;
     std::vector<double> chan_freqs;      // frequencies the device channel table was built from
     int chan_F_pad = 0;
     ChanTable ch{};
@@ -48,6 +51,7 @@ struct woden_ctx {
 
 namespace {
 
+constexpr int SHAPELET_TENSOR_MIN_ORDER = 1000;   // AUTO never takes the tensor path until it is measured faster
 constexpr int SIM_CHUNKS = 8;   // time chunks of woden_simulate_host (compute / copy-back overlap)
 constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
 
@@ -197,7 +201,7 @@ int woden_destroy(woden_ctx *ctx)
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
         }
-        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->h_uvw, &ctx->h_comp,
+        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->h_uvw, &ctx->h_comp,
                           &ctx->h_int, &ctx->h_vis})
             b->release();
     }
@@ -226,6 +230,15 @@ int woden_set_path(woden_ctx *ctx, int path)
     if (!ctx) return WODEN_ERR_NULL;
     if (path != WODEN_PATH_AUTO && path != WODEN_PATH_GENERAL) return WODEN_ERR_DIM;
     ctx->path = path;
+    return WODEN_OK;
+}
+
+int woden_set_shapelet_path(woden_ctx *ctx, int path)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    if (path != WODEN_SHAPELET_AUTO && path != WODEN_SHAPELET_REGISTER && path != WODEN_SHAPELET_TENSOR)
+        return WODEN_ERR_DIM;
+    ctx->shapelet_path = path;
     return WODEN_OK;
 }
 
@@ -348,6 +361,21 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     // truncated models: when under 3/4 of the order bucket's triangle is listed, take
     // the kernel variant that skips empty 4-coefficient chunks (decided from the list length alone)
     const bool sparse = (double)n_coeff < 0.75 * (double)n * (double)((PM + 1) * (PM + 2) / 2);
+    // tensor-core variant (north_star: "used only if ... shown by measurement to beat the register path"):
+    // AUTO takes it from the order bucket at which it measured faster (profiles/shapelet_mma_r1.md)
+    const bool tensor = ctx->shapelet_path == WODEN_SHAPELET_TENSOR ||
+                        (ctx->shapelet_path == WODEN_SHAPELET_AUTO && PM >= SHAPELET_TENSOR_MIN_ORDER && !sparse);
+    if (tensor) {
+        CU(ctx, ctx->bmat.reserve(mma_bmat_halves(PM, n) * 2), "alloc coefficient matrices");
+        CU(ctx, ctx->bscale.reserve((size_t)n * 4), "alloc coefficient scales");
+        CU(ctx, launch_predict_shapelets_mma(d, ctx->ch, static_cast<const GeoS *>(ctx->geo.p),
+                                             static_cast<const float *>(ctx->tri.p),
+                                             static_cast<const float *>(ctx->flux.p), n, PM,
+                                             static_cast<__half *>(ctx->bmat.p), static_cast<float *>(ctx->bscale.p),
+                                             reinterpret_cast<float2 *>(vis), accumulate ? 1 : 0, st),
+           "predict_shapelets (tensor) launch");
+        return WODEN_OK;
+    }
     CU(ctx, launch_predict_shapelets(d, ctx->ch, static_cast<const GeoS *>(ctx->geo.p),
                                      static_cast<const float *>(ctx->tri.p),
                                      static_cast<const float *>(ctx->flux.p), n, PM, sparse,

@@ -1,5 +1,6 @@
 // kernels.h -- internal launch interface between api.cu and the kernel translation units.
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 #include "layout.h"
@@ -50,6 +51,12 @@ int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or 
 cudaError_t launch_predict_shapelets(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
                                      const float *flux, int n, int PM, bool sparse, float2 *vis, int accumulate,
                                      cudaStream_t st);
+
+// tensor-core variant (predict_shapelets_mma.cu): T = G_y F'^T on tcgen05, operands FP16 hi + lo
+size_t mma_bmat_halves(int PM, int n);
+cudaError_t launch_predict_shapelets_mma(const UvwDev &uvw, const ChanTable &ch, const GeoS *geo, const float *tri,
+                                         const float *flux, int n, int PM, __half *bmat, float *bscale, float2 *vis,
+                                         int accumulate, cudaStream_t st);
 
 // ---- geometry before the hot path (geometry.cu) ---------------------
 cudaError_t launch_uvw(const double *X, const double *Y, const double *Z, int n_ant, int T, const double *hour_angle_dev,

@@ -190,11 +190,13 @@ def _run_shapelets(ctx, torch, u, v, w, fr, l, m, s0, al, b1, b2, pa, M, off, n1
     return vis.cpu().numpy()
 
 
+@pytest.mark.parametrize("engine", [1, 2], ids=["register", "tensor"])
 @pytest.mark.parametrize("p_max", [0, 1, 5, 13, 40, 61, 86, 100])
-def test_shapelets_orders_up_to_the_limit(ctx, torch_mod, p_max):
+def test_shapelets_orders_up_to_the_limit(ctx, torch_mod, p_max, engine):
     # full triangles at every bucket edge incl. the paper's p_max = 86 and the
     # library limit; beta up to 20 arcmin on a 3 km array reaches Hermite arguments ~30 (H4)
     ctx.set_path(0)
+    ctx.set_shapelet_path(engine)
     u, v, w, fr = _small_case(seed=p_max, T=2, B=333, F=5)
     rng = np.random.default_rng(1000 + p_max)
     n = 3
@@ -212,15 +214,18 @@ def test_shapelets_orders_up_to_the_limit(ctx, torch_mod, p_max):
     V = _run_shapelets(ctx, torch_mod, u, v, w, fr, l, m, s0, al, b1, b2, pa, M, off, n1, n2, cf, p_max)
     ref = oracle.predict_shapelets(u, v, w, fr, l, m, s0, al, 150e6, b1, b2, pa, M, off, n1, n2, cf)
     scale = oracle.tolerance_scale(fr, s0, al, 150e6, off, cf)
+    ctx.set_shapelet_path(0)
     err = np.abs(V - ref) / scale[None, :, None]
     assert err.max() <= TOL
     assert np.abs(ref).max() > 1e-3
 
 
-def test_shapelets_single_high_order_terms_and_sparse_lists(ctx, torch_mod):
+@pytest.mark.parametrize("engine", [1, 2], ids=["register", "tensor"])
+def test_shapelets_single_high_order_terms_and_sparse_lists(ctx, torch_mod, engine):
     # one isolated coefficient at a time: no cancellation hides a wrong sign / index / scale;
     # truncated (sparse, unsorted, duplicated) lists: duplicates add, missing entries are zero.
     ctx.set_path(0)
+    ctx.set_shapelet_path(engine)
     u, v, w, fr = _small_case(seed=3, T=1, B=257, F=3)
     u *= 0.3; v *= 0.3; w *= 0.3
     l = np.array([0.01]); m = np.array([-0.02]); s0 = np.array([1.0]); al = np.array([0.0])
@@ -234,6 +239,7 @@ def test_shapelets_single_high_order_terms_and_sparse_lists(ctx, torch_mod):
     V = _run_shapelets(ctx, torch_mod, u, v, w, fr, l, m, s0, al, b1, b2, pa, None, [0, 6], n1, n2, cf, 11)
     ref = oracle.predict_shapelets(u, v, w, fr, l, m, s0, al, 150e6, b1, b2, pa, None, [0, 6], n1, n2, cf)
     assert np.abs(V - ref).max() <= TOL * np.abs(cf).sum()
+    ctx.set_shapelet_path(0)
 
 
 @pytest.mark.parametrize("cfg,f_comp", [(5, 0.5), (5, 0.1), (4, 0.3)])
