@@ -51,7 +51,7 @@ struct woden_ctx {
 
 namespace {
 
-constexpr int SHAPELET_TENSOR_MIN_ORDER = 1000;   // AUTO never takes the tensor path until it is measured faster
+constexpr int SHAPELET_TENSOR_MIN_ORDER = 40;   // order bucket from which the tensor path measured faster
 constexpr int SIM_CHUNKS = 8;   // time chunks of woden_simulate_host (compute / copy-back overlap)
 constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
 
@@ -364,7 +364,7 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     // tensor-core variant (north_star: "used only if ... shown by measurement to beat the register path"):
     // AUTO takes it from the order bucket at which it measured faster (profiles/shapelet_mma_r1.md)
     const bool tensor = ctx->shapelet_path == WODEN_SHAPELET_TENSOR ||
-                        (ctx->shapelet_path == WODEN_SHAPELET_AUTO && PM >= SHAPELET_TENSOR_MIN_ORDER && !sparse);
+                        (ctx->shapelet_path == WODEN_SHAPELET_AUTO && PM >= SHAPELET_TENSOR_MIN_ORDER);
     if (tensor) {
         CU(ctx, ctx->bmat.reserve(mma_bmat_halves(PM, n) * 2), "alloc coefficient matrices");
         CU(ctx, ctx->bscale.reserve((size_t)n * 4), "alloc coefficient scales");

@@ -244,6 +244,7 @@ def test_shapelets_single_high_order_terms_and_sparse_lists(ctx, torch_mod, engi
 
 @pytest.mark.parametrize("cfg,f_comp", [(5, 0.5), (5, 0.1), (4, 0.3)])
 def test_truncated_shapelet_models_take_the_sparse_kernel(ctx, torch_mod, cfg, f_comp):
+    ctx.set_shapelet_path(1)        # register engine: its chunk-skipping variant is what this test is about
     # PAPER.md section 5.3 (Eq 23-24): basis functions ranked by absolute flux, a fraction kept; the
     # ragged coefficient lists go through the chunk-skipping kernel variant (PM = 40 NV = 2, PM = 60)
     from paper_2005_09316_b200 import truncate
@@ -258,8 +259,13 @@ def test_truncated_shapelet_models_take_the_sparse_kernel(ctx, torch_mod, cfg, f
     ref = oracle.predict_shapelets(u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, 150e6, s.beta1_rad, s.beta2_rad,
                                    s.pa_rad, s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff)
     scale = oracle.tolerance_scale(fr, s.s0_jy, s.alpha, 150e6, s.coeff_offset, s.coeff)
+    ctx.set_shapelet_path(0)
     assert (np.abs(V - ref) / scale[None, :, None]).max() <= TOL
     assert np.abs(ref).max() > 1e-3
+    # AUTO (tensor engine from order bucket 40) must agree as well
+    V2 = _run_shapelets(ctx, torch_mod, u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, s.beta1_rad, s.beta2_rad, s.pa_rad,
+                        s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff, pmax)
+    assert (np.abs(V2 - ref) / scale[None, :, None]).max() <= TOL
 
 
 def test_accumulate_zero_components_and_additivity(ctx, torch_mod):
