@@ -45,6 +45,7 @@ CONFIG_NAMES = {
     3: "Gaussian-heavy sky",
     4: "Fornax-A-like shapelet model",
     5: "Full-band mixed sky",
+    6: "Phase-II-like shapelet model (extra: SURVEY.md 8(f) NEXT-2)",
 }
 
 
@@ -239,7 +240,7 @@ def _array(rng, which: str):
     if which == "A32":
         return disk_antennas(rng, 32, 500.0)
     e1, n1 = disk_antennas(rng, 64, 100.0)
-    e2, n2 = disk_antennas(rng, 64, 1500.0)
+    e2, n2 = disk_antennas(rng, 64, 2750.0 if which == "A128L" else 1500.0)
     return np.concatenate([e1, e2]), np.concatenate([n1, n2])
 
 
@@ -249,6 +250,9 @@ _OBS = {  # config: (array, T, dt_s, F)
     3: ("A128", 14, 8.0, 32),
     4: ("A128", 14, 8.0, 384),
     5: ("A128", 56, 2.0, 384),
+    # not a BASELINE.json config: the 5.5 km phase II-like array with the paper's p_max = 86 lobes
+    # (PAPER.md:171, :183), the sixth case SURVEY.md 8(f) NEXT-2 suggests
+    6: ("A128L", 14, 8.0, 384),
 }
 
 
@@ -258,7 +262,7 @@ def make_antennas(config: int, *, t_index0: int = 0, n_times_total: Optional[int
     (X, Y, Z) in metres [n_ant], hour angles [T] in radians, and the phase-centre declination --
     the inputs of woden_uvw_from_antennas.  Same draws as make_config."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..5, got {config}")
+        raise ValueError(f"config must be 1..6, got {config}")
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + config))
     arr, T, dt, _ = _OBS[config]
     if n_times is None:
@@ -275,7 +279,7 @@ def make_antennas(config: int, *, t_index0: int = 0, n_times_total: Optional[int
 def make_config_shape(config: int):
     """(array name, T, dt_s, F) of config 1..5 without generating it."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..5, got {config}")
+        raise ValueError(f"config must be 1..6, got {config}")
     return _OBS[config]
 
 
@@ -285,7 +289,7 @@ def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] 
     longer observation with the same sky and array (weak-scaling ranks, SURVEY.md §8(e));
     the defaults give the config exactly as BASELINE.json words it."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..5, got {config}")
+        raise ValueError(f"config must be 1..6, got {config}")
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + config))
     arr, T, dt, F = _OBS[config]
     if n_times is None:
@@ -324,6 +328,9 @@ def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] 
                          alpha=alpha[:n_pt].copy())
         gau = Components(l=l[n_pt:].copy(), m=m[n_pt:].copy(), s0_jy=s0[n_pt:].copy(),
                          alpha=alpha[n_pt:].copy(), maj_fwhm_rad=maj, min_fwhm_rad=mnr, pa_rad=pa)
+    elif config == 6:
+        cl = np.array([-np.sin(np.deg2rad(0.25)), np.sin(np.deg2rad(0.25))])
+        shp = _shapelets(rng, cl, np.zeros(2), 86, 5.0, 20.0)
     elif config == 5:
         pts = _points(rng, 8000, 25.0, 0.01, 10.0)
         gau = _gaussians(rng, 2000, 25.0, 0.01, 10.0, 1.0, 30.0)
