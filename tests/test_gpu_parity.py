@@ -268,6 +268,45 @@ def test_truncated_shapelet_models_take_the_sparse_kernel(ctx, torch_mod, cfg, f
     assert (np.abs(V2 - ref) / scale[None, :, None]).max() <= TOL
 
 
+def test_tensor_engine_accumulates_and_handles_ragged_batches(ctx, torch_mod):
+    # the tcgen05 engine owns 128 visibilities per CTA: T x B = 3 x 171 = 513 leaves a one-row tail;
+    # accumulate = 1 must add into the buffer; two identical calls must be bit-identical
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(0)
+    u, v, w, fr = _small_case(seed=44, T=3, B=171, F=4)
+    rng = np.random.default_rng(44)
+    n, p_max = 2, 44
+    l, m = inputs.disk_lm(rng, n, 8.0)
+    s0 = np.array([1.5, -0.7]); al = np.array([-0.8, -0.3])
+    b1 = np.array([6.0, 15.0]) * inputs.ARCMIN; b2 = np.array([9.0, 4.0]) * inputs.ARCMIN
+    pa = rng.uniform(0, np.pi, n)
+    t1, t2 = inputs.full_triangle(p_max)
+    P = len(t1)
+    n1 = np.tile(t1, n); n2 = np.tile(t2, n)
+    cf = rng.normal(0, 1, n * P) * np.exp(-(n1 + n2) / 10.0) * 1e3        # large coefficients: exercises the scaling
+    off = np.arange(n + 1) * P
+    d = lambda a: _dev(torch, a)
+    di = lambda a: _dev(torch, a, torch.int32)
+    uvw = binding.Uvw(d(u), d(v), d(w), fr)
+    args = (uvw, d(l), d(m), d(s0), d(al), 150e6, d(b1), d(b2), d(pa), None, di(off), len(cf), p_max, di(n1), di(n2), d(cf))
+    ctx.set_shapelet_path(2)
+    base = torch.full(uvw.vis_shape, 2 - 3j, dtype=torch.complex64, device="cuda:0")
+    acc = base.clone()
+    ctx.predict_shapelets(*args, acc, True)
+    plain = ctx.new_vis(uvw)
+    ctx.predict_shapelets(*args, plain, False)
+    again = ctx.new_vis(uvw)
+    ctx.predict_shapelets(*args, again, False)
+    torch.cuda.synchronize(); ctx.check()
+    ctx.set_shapelet_path(0)
+    assert torch.equal(plain, again)
+    assert torch.max(torch.abs(acc - (base + plain))).item() <= 1e-3 * float(torch.max(torch.abs(plain)).item()) * 1e-3
+    ref = oracle.predict_shapelets(u, v, w, fr, l, m, s0, al, 150e6, b1, b2, pa, None, off, n1, n2, cf)
+    scale = oracle.tolerance_scale(fr, s0, al, 150e6, off, cf)
+    assert (np.abs(plain.cpu().numpy() - ref) / scale[None, :, None]).max() <= TOL
+
+
 def test_accumulate_zero_components_and_additivity(ctx, torch_mod):
     from paper_2005_09316_b200 import binding
     torch = torch_mod
