@@ -37,7 +37,7 @@ SM_COUNT = 148
 MUFU_LANES_PER_SM = 16          # measured: profiles/pipes_r1.md
 FP32_LANES_PER_SM = 128
 SM_MAX_HZ = 1965e6
-LAUNCHES_PER_STEP = {"points": 3, "gaussians": 3, "shapelets": 5}   # pack + predict kernels
+LAUNCHES_PER_STEP = {"points": 3, "gaussians": 3, "shapelets": 6}   # pack + predict kernels (+1: tensor engine)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on config 5 (profiles/ncu_r1_kernels.md)
 NCU_DRAM_BYTES = {("points", "walk"): 158166016 + 1345318912, ("gaussians", "walk"): 1536168960 + 1339894272,
                   ("shapelets", "walk"): 1419681792 + 1340600320, ("shapelets", "general"): 1419681792 + 1340600320}
@@ -335,6 +335,8 @@ def run_ours(args):
 
     launches = args.steps * sum(LAUNCHES_PER_STEP[k] for k in ("points", "gaussians", "shapelets")
                                 if counts[k] > 0)
+    if counts["shapelets"] > 0 and int((wl.shapelets.n1 + wl.shapelets.n2).max()) > 32:
+        launches += args.steps              # order bucket >= 40: tensor engine stages its FP16 coefficient matrices
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
