@@ -340,9 +340,10 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32 accumulate, f64 phase", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": config_dict(wl, {
             "path": "auto (channel walking: uniform 80 kHz channels)" if walk else "general",
+            "arithmetic": "FP32 sums and phasors, FP64 phase before reduction to its fraction; complex64 output",
             "l2": "no flush: each step writes 1.4 GB of visibilities, 11x the 126 MB L2; component blocks "
                   "are meant to be L2 resident",
             "parallelism": "1 GPU" if world == 1 else f"time-sharded x{world}, no collective"}),
@@ -427,6 +428,66 @@ def run_truncation(args):
     return 0
 
 
+def run_only(args):
+    """One C-ABI predict call of one component type on the config's grid (what the per-kernel ncu
+    captures under profiles/ run): `--only points|gaussians|shapelets`, optionally the first
+    `--max-components` components, for shapelets optionally full triangles of `--shapelet-order`
+    (the config's decay law, seed 1) and a forced `--shapelet-engine`.  Prints one JSON line."""
+    import torch
+    from paper_2005_09316_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --only: no CUDA device")
+    wl = inputs.make_config(args.config)
+    ctx = binding.Woden(0)
+    ctx.set_path(binding.WODEN_PATH_GENERAL if args.path == "general" else binding.WODEN_PATH_AUTO)
+    ctx.set_shapelet_path({"auto": 0, "register": 1, "tensor": 2}[args.shapelet_engine])
+    dev = lambda a, dt=torch.float64: torch.as_tensor(np.ascontiguousarray(a), dtype=dt, device="cuda:0")
+    uvw = binding.Uvw(dev(wl.u_m), dev(wl.v_m), dev(wl.w_m), wl.freqs_hz)
+    vis = ctx.new_vis(uvw)
+    n_max = args.max_components if args.max_components > 0 else None
+    if args.only == "points":
+        p = wl.points
+        a = [dev(x[:n_max]) for x in (p.l, p.m, p.s0_jy, p.alpha)]
+        call = lambda: ctx.predict_points(uvw, *a, wl.ref_freq_hz, vis, False)
+        units, unit_name = int(a[0].numel()), "components"
+    elif args.only == "gaussians":
+        g = wl.gaussians
+        a = [dev(x[:n_max]) for x in (g.l, g.m, g.s0_jy, g.alpha, g.maj_fwhm_rad, g.min_fwhm_rad, g.pa_rad)]
+        call = lambda: ctx.predict_gaussians(uvw, *a[:4], wl.ref_freq_hz, *a[4:], vis, False)
+        units, unit_name = int(a[0].numel()), "components"
+    else:
+        sh = wl.shapelets
+        n1, n2, cf, off = sh.n1, sh.n2, sh.coeff, sh.coeff_offset
+        if args.shapelet_order >= 0:
+            rng = np.random.default_rng(1)
+            t1, t2 = inputs.full_triangle(args.shapelet_order)
+            n1, n2 = np.tile(t1, sh.n), np.tile(t2, sh.n)
+            cf = rng.normal(0, 1, n1.size) * np.exp(-(n1 + n2) / 10.0)
+            off = np.arange(sh.n + 1) * len(t1)
+        a = [dev(x) for x in (sh.l, sh.m, sh.s0_jy, sh.alpha)]
+        b = [dev(x) for x in (sh.beta1_rad, sh.beta2_rad, sh.pa_rad, sh.uv_basis)]
+        i = [dev(x, torch.int32) for x in (off, n1, n2)]
+        c = dev(cf)
+        pmax = int((n1 + n2).max())
+        call = lambda: ctx.predict_shapelets(uvw, *a, wl.ref_freq_hz, *b, i[0], int(cf.size), pmax, i[1], i[2], c, vis,
+                                             False)
+        units, unit_name = int(cf.size), "coefficients"
+    for _ in range(max(1, args.warmup)):
+        call()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(max(1, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); call(); e1.record(); torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    ctx.check()
+    ms = float(np.median(ts))
+    print(json.dumps({"only": args.only, "config": args.config, unit_name: units, "n_vis": wl.n_vis, "path": args.path,
+                      "shapelet_engine": args.shapelet_engine, "ms": ms, "min_ms": float(min(ts)),
+                      f"{unit_name}_x_visibility_per_s": units * wl.n_vis / (ms * 1e-3)}))
+    return 0
+
+
 def run_peel(args):
     """The paper's consumer of the predicted visibilities (section 5.1): fit one complex gain
     per antenna and (time, frequency) cell by 10 passes of Eq 22, then subtract the calibrated model.
@@ -493,6 +554,11 @@ def main():
     ap.add_argument("--path", choices=["auto", "general"], default="auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipes", action="store_true", help="print the measured pipe rates and exit")
+    ap.add_argument("--only", choices=["points", "gaussians", "shapelets"], default=None,
+                    help="time ONE predict call of one component type (used for the per-kernel ncu captures) and exit")
+    ap.add_argument("--max-components", type=int, default=0, help="--only: use the first N components")
+    ap.add_argument("--shapelet-order", type=int, default=-1, help="--only shapelets: full triangles of this order")
+    ap.add_argument("--shapelet-engine", choices=["auto", "register", "tensor"], default="auto")
     ap.add_argument("--peel", action="store_true",
                     help="time the gain fit and peel of PAPER.md section 5.1 on the config and exit")
     ap.add_argument("--truncation", action="store_true",
@@ -502,6 +568,8 @@ def main():
         return run_pipes(args)
     if args.truncation:
         return run_truncation(args)
+    if args.only:
+        return run_only(args)
     if args.peel:
         return run_peel(args)
     if args.impl == "reference":
