@@ -84,6 +84,8 @@ def truncate_shapelets(s: Components, f_comp: float, weights: Optional[np.ndarra
     """Keep the basis functions Eq 23-24 select, ranked over ALL shapelet components together
     (the paper's N_tot counts basis functions of both lobes, :271).  Components are kept even
     when all their basis functions go (empty CSR range)."""
+    if s.n == 0 or s.coeff is None:
+        return s
     if weights is None:
         weights = shapelet_basis_weights(s)
     idx = keep_indices(weights, f_comp)

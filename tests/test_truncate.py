@@ -50,6 +50,8 @@ def test_shapelet_truncation_keeps_csr_consistent():
             assert np.array_equal(t.coeff, s.coeff)
         else:
             assert 0 < t.coeff.size < s.coeff.size
+    empty = inputs.make_config(2).shapelets                      # a config without shapelets passes through
+    assert truncate.truncate_shapelets(empty, 0.5).n == 0
     # the (0,0) weight is |C| * 1 by construction (pixel-sum normalisation of each component's basis)
     j0 = int(s.coeff_offset[0])
     assert s.n1[j0] == 0 and s.n2[j0] == 0
