@@ -1,13 +1,16 @@
 // predict_shapelets.cu -- step S6 (+S1, S3, S4, S7) of the hot path for shapelet components
 // (Eq 11 with the envelope of Eq 15-17; basis FT Eq 3, :60).
 //
-// Register path: one thread owns one visibility (b, t, f).  Per
-// shapelet it evaluates the scaled Hermite functions g_p(y) = h_p(y)/lam_p, p = 0..PM, into
+// Register engine (the tensor-core engine is predict_shapelets_mma.cu): one
+// thread owns NV visibilities, one (baseline, time) pair at NV consecutive channels.  Per shapelet
+// and visibility it evaluates the scaled Hermite functions g_p(y) = h_p(y)/lam_p, p = 0..PM, into
 // registers by the two-operation recurrence g_{p+1} = (c_p y) g_p - g_{p-1}, walks g_{n1}(x) on
 // the fly, and contracts the dense coefficient triangle, one FFMA per coefficient, with the
 // coefficients broadcast from shared memory (LDS.128 = 4 coefficients).  The triangle of each
 // shapelet is fetched by one bulk async copy (TMA engine) into shared memory.  The order PM is a
-// compile-time bucket so that every register index and shared-memory offset is static.
+// compile-time bucket so that every register index and shared-memory offset is static.  The
+// SPARSE variant (truncated models) skips the 4-coefficient chunks whose staged
+// mask bit is clear.
 //
 // i^(n1+n2) (reading G3): the sign part (-1)^floor(p/2) of each factor i^p is folded into the
 // stored coefficient by pack.cu, so even n2 add to E, odd n2 to O, and row n1 contributes
