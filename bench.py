@@ -488,6 +488,42 @@ def run_only(args):
     return 0
 
 
+def run_basis(args):
+    """NEXT-5 experiment: evaluate the 1-D shapelet series sum_p c_p h_p(x) for 2^26 arguments by the
+    recurrence of the predict kernels and by the paper's look-up tables; time and
+    maximum error against the oracle's long-double Hermite routine on a 4096-point sample."""
+    import torch
+    import oracle
+    from paper_2005_09316_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --basis: no CUDA device")
+    ctx = binding.Woden(0)
+    rng = np.random.default_rng(7)
+    n = 1 << 26
+    x = torch.empty(n, dtype=torch.float32, device="cuda:0").uniform_(-12.0, 12.0, generator=torch.Generator("cuda:0").manual_seed(7))
+    out = torch.empty_like(x)
+    rows = []
+    for pm in (40, 86):
+        c = (rng.normal(0, 1, pm + 1) * np.exp(-np.arange(pm + 1) / 10.0)).astype(np.float32)
+        cd = torch.as_tensor(c, device="cuda:0")
+        xs = x[:4096].cpu().numpy()
+        ref = np.array([np.dot(c.astype(np.float64), oracle.hermite_functions(pm, float(v))) for v in xs])
+        for name, method, dx in (("recurrence", 0, 0.0), ("lut dx=2^-7", 1, 2.0 ** -7), ("lut dx=2^-10", 1, 2.0 ** -10)):
+            call = lambda: ctx.shapelet_series(method, x, cd, lut_dx=dx or 1.0, lut_x_max=32.0, out=out)
+            call(); torch.cuda.synchronize()
+            ts = []
+            for _ in range(max(3, args.steps)):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); call(); e1.record(); torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            err = float(np.abs(out[:4096].cpu().numpy() - ref).max() / np.abs(c).sum())
+            table_mb = 0.0 if method == 0 else np.ceil(32.0 / dx) * (pm + 1) * 8 / 1e6
+            rows.append({"p_max": pm, "method": name, "ms": float(np.median(ts)), "basis_values_per_s": n * (pm + 1) / (np.median(ts) * 1e-3),
+                         "max_err_over_sum_abs_coeff": err, "table_MB": table_mb})
+    print(json.dumps({"basis": rows, "n_arguments": n}))
+    return 0
+
+
 def run_peel(args):
     """The paper's consumer of the predicted visibilities (section 5.1): fit one complex gain
     per antenna and (time, frequency) cell by 10 passes of Eq 22, then subtract the calibrated model.
@@ -559,6 +595,8 @@ def main():
     ap.add_argument("--max-components", type=int, default=0, help="--only: use the first N components")
     ap.add_argument("--shapelet-order", type=int, default=-1, help="--only shapelets: full triangles of this order")
     ap.add_argument("--shapelet-engine", choices=["auto", "register", "tensor"], default="auto")
+    ap.add_argument("--basis", action="store_true",
+                    help="look-up-table vs recurrence evaluation of the shapelet basis (PAPER.md:159) and exit")
     ap.add_argument("--peel", action="store_true",
                     help="time the gain fit and peel of PAPER.md section 5.1 on the config and exit")
     ap.add_argument("--truncation", action="store_true",
@@ -570,6 +608,8 @@ def main():
         return run_truncation(args)
     if args.only:
         return run_only(args)
+    if args.basis:
+        return run_basis(args)
     if args.peel:
         return run_peel(args)
     if args.impl == "reference":

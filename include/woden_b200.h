@@ -206,6 +206,19 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells,
                const float *vis_data, const float *vis_model, const double *gains,
                float *vis_out, void *cuda_stream);
 
+/* Basis-evaluation experiment: the 1-D shapelet series
+ *   out[i] = sum_{p <= p_max} coeff[p] h_p(x[i]),   h_p(x) = H_p(x) exp(-x^2/2)/sqrt(2^p p!)
+ * by the FP32 three-term recurrence of the predict kernels (WODEN_BASIS_RECURRENCE) or by the
+ * paper's mechanism: linear interpolation in one-dimensional look-up tables of
+ * h_p on the grid ix * lut_dx, 0 <= x < lut_x_max, built on the device in FP64 and cached in the
+ * context (WODEN_BASIS_LUT; error <= lut_dx^2 (2p+1) 1.09 / 8 per basis value; |x| beyond the
+ * table gives 0).  x, coeff ([p_max + 1]) and out: DEVICE float arrays, n values. */
+#define WODEN_BASIS_RECURRENCE 0
+#define WODEN_BASIS_LUT        1
+int woden_shapelet_series(woden_ctx *ctx, int method, int p_max, long long n, const float *x,
+                          const float *coeff, double lut_dx, double lut_x_max, float *out,
+                          void *cuda_stream);
+
 /* Pipe microbenchmarks used to MEASURE the roofline denominators.
  * Runs `which` (WODEN_PIPE_*) for `iters` dependent-chain-free iterations on every SM and
  * returns warp-instructions per second per GPU in *ops_per_s (thread-ops/s = x32) and the

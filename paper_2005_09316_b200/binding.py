@@ -29,13 +29,15 @@ WODEN_PATH_GENERAL = 1
 WODEN_SHAPELET_AUTO = 0
 WODEN_SHAPELET_REGISTER = 1
 WODEN_SHAPELET_TENSOR = 2
+WODEN_BASIS_RECURRENCE = 0
+WODEN_BASIS_LUT = 1
 PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA_IMM": 6, "F2F": 7,
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -90,6 +92,7 @@ def load() -> C.CDLL:
     L.woden_check.argtypes = [_vp]
     L.woden_set_path.argtypes = [_vp, C.c_int]
     L.woden_set_shapelet_path.argtypes = [_vp, C.c_int]
+    L.woden_shapelet_series.argtypes = [_vp, C.c_int, C.c_int, C.c_longlong, _vp, _vp, C.c_double, C.c_double, _vp, _vp]
     common = [_vp, C.POINTER(woden_uvw), C.c_int, _vp, _vp, _vp, _vp, C.c_double]
     tail = [_vp, C.c_int, _vp]
     L.woden_predict_points.argtypes = common + tail
@@ -306,6 +309,20 @@ class Woden:
         rc = self._L.woden_peel(self._ctx, int(n_antennas), cells, _ptr(vis_data), _ptr(vis_model), _ptr(gains),
                                 _ptr(out), _stream_handle(stream))
         self._ck(rc, "woden_peel")
+        return out
+
+    def shapelet_series(self, method: int, x, coeff, lut_dx: float = 2.0 ** -7, lut_x_max: float = 32.0, out=None,
+                        stream=None):
+        """sum_p coeff[p] h_p(x) for a float32 device tensor x (woden_shapelet_series)."""
+        import torch
+        if x.dtype != torch.float32 or coeff.dtype != torch.float32:
+            raise ValueError("x and coeff must be float32 device tensors")
+        if out is None:
+            out = torch.empty_like(x)
+        rc = self._L.woden_shapelet_series(self._ctx, int(method), int(coeff.numel()) - 1, int(x.numel()), _ptr(x),
+                                           _ptr(coeff), float(lut_dx), float(lut_x_max), _ptr(out),
+                                           _stream_handle(stream))
+        self._ck(rc, "woden_shapelet_series")
         return out
 
     def pipe_rate(self, which: str, iters: int = 20000):

@@ -38,7 +38,9 @@ struct woden_ctx {
     int path = WODEN_PATH_AUTO;
     cudaStream_t last_stream = nullptr;
     std::string last_error;
-    DevBuf geo, flux, tri, chan, err, hang, bmat, bscale;
+    DevBuf geo, flux, tri, chan, err, hang, bmat, bscale, lut;
+    int lut_pm = -1, lut_nx = 0;
+    double lut_dx = 0.0;
     int shapelet_path = WODEN_SHAPELET_AUTO;
     std::vector<double> chan_freqs;      // frequencies the device channel table was built from
     int chan_F_pad = 0;
@@ -201,7 +203,7 @@ int woden_destroy(woden_ctx *ctx)
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
         }
-        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->h_uvw, &ctx->h_comp,
+        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->lut, &ctx->h_uvw, &ctx->h_comp,
                           &ctx->h_int, &ctx->h_vis})
             b->release();
     }
@@ -593,6 +595,31 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells, const float *v
                         reinterpret_cast<const double2 *>(gains), reinterpret_cast<float2 *>(vis_out), n_antennas,
                         n_cells, st),
        "peel launch");
+    return WODEN_OK;
+}
+
+int woden_shapelet_series(woden_ctx *ctx, int method, int p_max, long long n, const float *x, const float *coeff,
+                          double lut_dx, double lut_x_max, float *out, void *cuda_stream)
+{
+    if (!ctx || !x || !coeff || !out) return WODEN_ERR_NULL;
+    if (p_max < 0 || p_max > WODEN_MAX_ORDER) return WODEN_ERR_ORDER;
+    if (n <= 0 || (method != WODEN_BASIS_RECURRENCE && method != WODEN_BASIS_LUT)) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    int n_x = 0;
+    if (method == WODEN_BASIS_LUT) {
+        if (!(lut_dx > 0.0) || !(lut_x_max > lut_dx) || lut_x_max / lut_dx > 1 << 22) return WODEN_ERR_DIM;
+        n_x = (int)std::ceil(lut_x_max / lut_dx);
+        if (ctx->lut_pm != p_max || ctx->lut_nx != n_x || ctx->lut_dx != lut_dx) {       // (re)build the table
+            CU(ctx, ctx->lut.reserve((size_t)n_x * (p_max + 1) * sizeof(float2)), "alloc look-up table");
+            CU(ctx, launch_lut_build(static_cast<float2 *>(ctx->lut.p), n_x, p_max, lut_dx, st), "table build launch");
+            ctx->lut_pm = p_max; ctx->lut_nx = n_x; ctx->lut_dx = lut_dx;
+        }
+    }
+    CU(ctx, launch_series(method, x, coeff, p_max, n, static_cast<const float2 *>(ctx->lut.p), n_x, lut_dx, out, st),
+       "series launch");
     return WODEN_OK;
 }
 

@@ -71,6 +71,11 @@ cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *g
 cudaError_t launch_peel(const float2 *data, const float2 *model, const double2 *gains, float2 *out, int N,
                         long long cells, cudaStream_t st);
 
+// ---- basis evaluation experiment: look-up table vs recurrence (basis_lut.cu)
+cudaError_t launch_lut_build(float2 *T, int n_x, int PM, double dx, cudaStream_t st);
+cudaError_t launch_series(int method, const float *x, const float *c, int PM, long long n, const float2 *T, int n_x,
+                          double dx, float *out, cudaStream_t st);
+
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
 
