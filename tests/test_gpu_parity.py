@@ -64,7 +64,7 @@ def test_config1_tiny_full_parity(ctx, path):
 
 
 @pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
-@pytest.mark.parametrize("cfg,n_random", [(2, 200_000), (3, 20_000), (4, 6_000), (5, 6_000), (6, 3_000)])
+@pytest.mark.parametrize("cfg,n_random", [(2, 200_000), (3, 20_000), (4, 60_000), (5, 100_000), (6, 20_000)])
 def test_configs_2_to_5_full_size_sampled_parity(ctx, cfg, n_random, path):
     wl = inputs.make_config(cfg)
     V = _gpu_total(ctx, wl, path)
