@@ -10,10 +10,11 @@ SHAPES = {  # config: (B, T, F, Kp, Kg, Ks, n_coeff)
     3: (8128, 14, 32, 0, 10000, 0, 0),
     4: (8128, 14, 384, 14340, 5660, 2, 2 * 1891),
     5: (8128, 56, 384, 8000, 2000, 4, 4 * 861),
+    6: (8128, 14, 384, 0, 0, 2, 2 * 3828),          # extra: phase II-like
 }
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5, 6])
 def test_config_shapes_and_preconditions(cfg):
     wl = inputs.make_config(cfg)
     B, T, F, Kp, Kg, Ks, P = SHAPES[cfg]
@@ -26,7 +27,7 @@ def test_config_shapes_and_preconditions(cfg):
             assert np.all(c.l ** 2 + c.m ** 2 < 1.0)
     # baseline lengths: |b| <= 2 * 1500 m (A128) or 2 * 500 m (A32), rotation preserves length
     blen = np.sqrt(wl.u_m ** 2 + wl.v_m ** 2 + wl.w_m ** 2)
-    assert blen.max() <= (1000.0 if cfg == 1 else 3000.0)
+    assert blen.max() <= {1: 1000.0, 6: 5500.0}.get(cfg, 3000.0)
     assert np.allclose(blen, blen[0][None, :], rtol=1e-12)
     if wl.gaussians.n:
         g = wl.gaussians
