@@ -33,6 +33,12 @@
  *
  * Output layout: complex64 interleaved (re, im), vis[((t * n_freqs) + f) * n_baselines + b].
  *
+ * Phase range: the phase u l + v m + w (n - 1) is formed in FP64 and reduced to its fraction to
+ * 2^-23 turn before the FP32 sin/cos, on every path (general, channel-walking, shapelets), as
+ * long as sqrt(2) |b| nu / c < 2^28 wavelengths for every baseline b = (u_m, v_m, w_m) and channel
+ * (a bound on the phase for l^2 + m^2 < 1).  The point / Gaussian kernels count baselines beyond
+ * that range for woden_check() (WODEN_ERR_DATA); their output is then undefined.
+ *
  * There is no CPU fallback anywhere: without a CUDA device every entry point that needs one
  * returns WODEN_ERR_CUDA.
  */
@@ -65,17 +71,27 @@ const char *woden_strerror(int status);
 const char *woden_last_error(const woden_ctx *ctx);
 
 /* Synchronises the context's last stream and reports device-side precondition violations
- * counted since the last check (l^2+m^2 >= 1, non-finite parameters, beta <= 0, shapelet
- * orders above p_max): WODEN_OK or WODEN_ERR_DATA.  Not on the hot path. */
+ * counted since the last check (l^2+m^2 >= 1, non-finite parameters, a flux s0 (nu/ref)^alpha that
+ * is not finite in FP32 at any channel, negative widths, beta <= 0, shapelet orders above p_max,
+ * baselines beyond the phase range above): WODEN_OK or WODEN_ERR_DATA.  Not on the hot path. */
 int woden_check(woden_ctx *ctx);
 
 /* Algorithm selection (measurement / testing).  Default WODEN_PATH_AUTO.
- *   AUTO    : channel-walking fast path when freqs_hz is uniformly spaced, else general
+ *   AUTO    : channel-walking fast path when freqs_hz is an arithmetic progression (to 1e-9 of
+ *             the step) of >= 8 channels whose step is at most 1/64 of the lowest frequency of
+ *             the list continued to a multiple of 32 channels (so that a 16-channel chain spans
+ *             at most +-12.5 % in frequency); otherwise the general path
  *   GENERAL : always one sin/cos (and one exp2 for Gaussians) per component x visibility
- * Both meet the same parity tolerance. */
+ * Both meet the same parity tolerance and the same phase range. */
 #define WODEN_PATH_AUTO    0
 #define WODEN_PATH_GENERAL 1
 int woden_set_path(woden_ctx *ctx, int path);
+/* Which point / Gaussian kernel family the last woden_predict_points / _gaussians call on this
+ * context launched: WODEN_PATH_GENERAL, WODEN_PATH_WALKING, or WODEN_PATH_NONE (n == 0 / no call
+ * yet).  For tests and reports; never changes behaviour. */
+#define WODEN_PATH_NONE    -1
+#define WODEN_PATH_WALKING 2
+int woden_last_path(const woden_ctx *ctx);
 
 /* Shapelet engine selection (measurement / testing).  Default WODEN_SHAPELET_AUTO.
  *   REGISTER : FP32 register path, one FFMA per coefficient (predict_shapelets.cu)
@@ -220,14 +236,25 @@ int woden_shapelet_series(woden_ctx *ctx, int method, int p_max, long long n, co
                           void *cuda_stream);
 
 /* Pipe microbenchmarks used to MEASURE the roofline denominators.
- * Runs `which` (WODEN_PIPE_*) for `iters` dependent-chain-free iterations on every SM and
- * returns warp-instructions per second per GPU in *ops_per_s (thread-ops/s = x32) and the
- * SM clock in Hz observed by clock64 over the run in *sm_clock_hz.  Synchronous. */
-#define WODEN_PIPE_FFMA   0
-#define WODEN_PIPE_MUFU   1   /* sin.approx + cos.approx + ex2.approx mix on the XU pipe */
-#define WODEN_PIPE_DFMA   2
-#define WODEN_PIPE_I2F    3
-#define WODEN_PIPE_LOP3   4
+ * Runs pattern `which` (WODEN_PIPE_*) for `iters` loop iterations of 16 independent register
+ * chains per thread on every SM (2 CTAs of 512 threads each) and returns, for the whole GPU, the
+ * rate of the counted operation in THREAD-operations per second in *thread_ops_per_s (one FFMA2
+ * counts as two FMAs; warp-instructions/s = that / 32) and the SM clock in Hz observed by
+ * clock64 against the global timer in *sm_clock_hz.  Synchronous (default stream). */
+#define WODEN_PIPE_FFMA         0   /* FFMA, a = a b + c with b, c fixed (operand-reuse cache hits)  */
+#define WODEN_PIPE_MUFU         1   /* sin.approx + cos.approx mix on the XU pipe                    */
+#define WODEN_PIPE_DFMA         2
+#define WODEN_PIPE_I2F          3
+#define WODEN_PIPE_LOP3         4
+#define WODEN_PIPE_FFMA2        5   /* packed fma.rn.f32x2, operands as in FFMA; counts 2 FMAs each  */
+#define WODEN_PIPE_FFMA_IMM     6   /* FFMA with immediate multiplier and addend                     */
+#define WODEN_PIPE_F2F          7   /* F2F.F32.F64 conversions                                       */
+#define WODEN_PIPE_MUFU_EX2     8   /* ex2.approx only                                               */
+#define WODEN_PIPE_MUFU_FFMA    9   /* 2 MUFU + 12 FFMA interleaved; counts the MUFUs                */
+#define WODEN_PIPE_FFMA_3REG   10   /* FFMA with three distinct, changing register operands          */
+#define WODEN_PIPE_FFMA2_3REG  11   /* FFMA2 with three distinct, changing register pairs            */
+#define WODEN_PIPE_FFMA2_BCAST 12   /* FFMA2 with one fixed pair and two changing pairs              */
+#define WODEN_PIPE_COUNT       13
 int woden_pipe_rate(woden_ctx *ctx, int which, int iters, double *thread_ops_per_s,
                     double *sm_clock_hz);
 

@@ -26,6 +26,8 @@ WODEN_ERR_DATA = -6
 WODEN_MAX_ORDER = 100
 WODEN_PATH_AUTO = 0
 WODEN_PATH_GENERAL = 1
+WODEN_PATH_NONE = -1
+WODEN_PATH_WALKING = 2
 WODEN_SHAPELET_AUTO = 0
 WODEN_SHAPELET_REGISTER = 1
 WODEN_SHAPELET_TENSOR = 2
@@ -35,7 +37,7 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
-           "woden_set_path", "woden_predict_points", "woden_predict_gaussians",
+           "woden_set_path", "woden_last_path", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
            "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series"]
 
@@ -91,6 +93,7 @@ def load() -> C.CDLL:
     L.woden_last_error.restype = C.c_char_p
     L.woden_check.argtypes = [_vp]
     L.woden_set_path.argtypes = [_vp, C.c_int]
+    L.woden_last_path.argtypes = [_vp]
     L.woden_set_shapelet_path.argtypes = [_vp, C.c_int]
     L.woden_shapelet_series.argtypes = [_vp, C.c_int, C.c_int, C.c_longlong, _vp, _vp, C.c_double, C.c_double, _vp, _vp]
     common = [_vp, C.POINTER(woden_uvw), C.c_int, _vp, _vp, _vp, _vp, C.c_double]
@@ -191,6 +194,9 @@ class Woden:
 
     def set_path(self, path: int):
         self._ck(self._L.woden_set_path(self._ctx, int(path)), "woden_set_path")
+
+    def last_path(self) -> int:
+        return int(self._L.woden_last_path(self._ctx))
 
     def set_shapelet_path(self, path: int):
         self._ck(self._L.woden_set_shapelet_path(self._ctx, int(path)), "woden_set_shapelet_path")

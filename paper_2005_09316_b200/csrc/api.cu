@@ -36,6 +36,7 @@ struct DevBuf {
 struct woden_ctx {
     int device = 0;
     int path = WODEN_PATH_AUTO;
+    int last_path = WODEN_PATH_NONE;
     cudaStream_t last_stream = nullptr;
     std::string last_error;
     DevBuf geo, flux, tri, chan, err, hang, bmat, bscale, lut;
@@ -56,6 +57,7 @@ namespace {
 constexpr int SHAPELET_TENSOR_MIN_ORDER = 40;   // order bucket from which the tensor path measured faster
 constexpr int SIM_CHUNKS = 8;   // time chunks of woden_simulate_host (compute / copy-back overlap)
 constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
+constexpr int WALK_MIN_F = 8;   // shorter channel lists take the general path
 
 int fail_cuda(woden_ctx *ctx, cudaError_t e, const char *where)
 {
@@ -107,13 +109,21 @@ int ensure_chan(woden_ctx *ctx, const woden_uvw *uvw, cudaStream_t st)
         s[f] = nu[f] / C_LIGHT;
         ns2[f] = (float)(-(s[f] * s[f]));
     }
+    // Channel-walking eligibility: an arithmetic progression (to 1e-9 of the step) of at least
+    // WALK_MIN_F channels whose continuation over the padded tiles stays positive and whose chains
+    // (seed +- 8 steps) span at most +-12.5 % in frequency.  The last condition is what keeps the
+    // Gaussian envelope walk exact where its seed has flushed to zero (predict_walk.cu) and keeps
+    // short, widely spaced lists (which would mostly fill the 32-channel tiles with padding) on the
+    // general path.
     int uniform = 0;
     double ds = 0.0;
-    if (F >= 2) {
+    if (F >= WALK_MIN_F) {
         const double d = uvw->freqs_hz[1] - uvw->freqs_hz[0];
         uniform = d != 0.0;
         for (int f = 0; f < F && uniform; ++f)
             if (std::fabs(uvw->freqs_hz[f] - (uvw->freqs_hz[0] + f * d)) > 1e-9 * std::fabs(d)) uniform = 0;
+        const double nu_lo = std::fmin(uvw->freqs_hz[0], uvw->freqs_hz[0] + (F_pad - 1) * d);
+        if (!(nu_lo > 0.0) || (WALK_FT / 4) * std::fabs(d) > 0.125 * nu_lo) uniform = 0;
         ds = d / C_LIGHT;
     }
     // the channel-walking kernel seeds its chains at fixed tile positions, which may lie past F in
@@ -235,6 +245,8 @@ int woden_set_path(woden_ctx *ctx, int path)
     return WODEN_OK;
 }
 
+int woden_last_path(const woden_ctx *ctx) { return ctx ? ctx->last_path : WODEN_PATH_NONE; }
+
 int woden_set_shapelet_path(woden_ctx *ctx, int path)
 {
     if (!ctx) return WODEN_ERR_NULL;
@@ -267,11 +279,13 @@ int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const doub
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ctx->last_stream = st;
+    ctx->last_path = WODEN_PATH_NONE;
     if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
     if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
     if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
     const int n_pad = (n + KB - 1) / KB * KB;
     const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    ctx->last_path = walk ? WODEN_PATH_WALKING : WODEN_PATH_GENERAL;
     const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoP)), "alloc geometry");
     CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
@@ -284,8 +298,8 @@ int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const doub
     const GeoP *geo = static_cast<const GeoP *>(ctx->geo.p);
     const float *flux = static_cast<const float *>(ctx->flux.p);
     float2 *out = reinterpret_cast<float2 *>(vis);
-    CU(ctx, walk ? launch_walk_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st)
-                 : launch_predict_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st),
+    CU(ctx, walk ? launch_walk_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st)
+                 : launch_predict_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st),
        "predict_points launch");
     return WODEN_OK;
 }
@@ -302,11 +316,13 @@ int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ctx->last_stream = st;
+    ctx->last_path = WODEN_PATH_NONE;
     if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
     if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
     if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
     const int n_pad = (n + KB - 1) / KB * KB;
     const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
+    ctx->last_path = walk ? WODEN_PATH_WALKING : WODEN_PATH_GENERAL;
     const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoG)), "alloc geometry");
     CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
@@ -320,8 +336,8 @@ int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     const GeoG *geo = static_cast<const GeoG *>(ctx->geo.p);
     const float *flux = static_cast<const float *>(ctx->flux.p);
     float2 *out = reinterpret_cast<float2 *>(vis);
-    CU(ctx, walk ? launch_walk_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st)
-                 : launch_predict_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, st),
+    CU(ctx, walk ? launch_walk_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st)
+                 : launch_predict_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st),
        "predict_gaussians launch");
     return WODEN_OK;
 }

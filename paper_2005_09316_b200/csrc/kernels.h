@@ -35,16 +35,16 @@ void launch_pack_coeffs(const int *coeff_offset, const int *n1, const int *n2, c
 // general path (predict_pg.cu): any channel list, one sin/cos (+ one exp2) per eval
 constexpr int PG_FT = 16;        // channels per thread
 cudaError_t launch_predict_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st);
+                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st);
 cudaError_t launch_predict_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo,
                                      const float *flux, int n_pad, float2 *vis, int accumulate,
-                                     cudaStream_t st);
+                                     unsigned int *err, cudaStream_t st);
 // channel-walking path (predict_walk.cu): equally spaced channels only
 constexpr int WALK_FT = 32;      // channels per thread: two chains of 16
 cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                               int n_pad, float2 *vis, int accumulate, cudaStream_t st);
+                               int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st);
 cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st);
+                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st);
 
 constexpr int SH_FT = 1;         // flux table tile for shapelets: [F][n] layout
 int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or -1

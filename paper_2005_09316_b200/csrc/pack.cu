@@ -89,8 +89,9 @@ __global__ void pack_flux_kernel(const double *__restrict__ s0, const double *__
     float val = 0.f;
     if (k < n && f < F) {
         const double v = s0[k] * pow(nu[f] * inv_ref, alpha[k]);
-        if (isfinite(v)) val = (float)v;
-        else if (j == 0) atomicAdd(err, 1u);
+        // FP32 table: a flux that is not finite (or overflows FP32) is replaced by 0 and counted
+        if (isfinite(v) && fabs(v) <= 3.4028234663852886e38) val = (float)v;
+        else atomicAdd(err, 1u);
     }
     flux[i] = val;
 }

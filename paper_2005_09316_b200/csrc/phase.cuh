@@ -8,6 +8,21 @@ namespace woden {
 
 constexpr double MAGIC23 = 805306368.0;  // 1.5 * 2^29 : ulp of the sum = 2^-23 turn
 constexpr double MAGIC32 = 1572864.0;    // 1.5 * 2^20 : low word of the sum = frac as Q0.32
+// Range of the two hand-offs.  phi + MAGIC23 stays in its binade while |phi| < 2^28 turns.  The
+// Q0.32 form needs |phi| < 2^19 turns for MAGIC32 itself; with the magic constant 1.5*2^(20+k) the
+// low word holds phi modulo 2^k turns in units of 2^(k-32) turn, and `<< k` leaves the fraction
+// with k fewer bits -- at k = 9 the same 2^28 turns / 2^-23 turn as MAGIC23.
+constexpr int PHASE_MAX_SHIFT = 9;
+// smallest k with bound < 2^(19+k) (bound >= 0; returns > PHASE_MAX_SHIFT when out of range)
+__device__ __forceinline__ int phase_shift_for(double bound)
+{
+    const int e = (__double2hiint(bound) >> 20) - 1023;         // floor(log2(bound)) for normal values
+    return e >= 19 ? e - 18 : 0;
+}
+__device__ __forceinline__ double magic32_shifted(int k)
+{
+    return __hiloint2double(0x41380000 + (k << 20), 0);          // 1.5 * 2^(20 + k)
+}
 constexpr float TWO_PI_F = 6.283185307179586f;
 constexpr float THREE_PI_F = 9.42477796076938f;
 constexpr float Q32_TO_RAD = 1.4629180792671596e-09f;   // 2 pi / 2^32

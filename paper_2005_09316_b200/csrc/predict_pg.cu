@@ -35,6 +35,7 @@ struct PGParams {
     float2 *vis;                     // [T][F][B]
     long long n_bt;                  // T * B
     int B, F, n_pad, accumulate;
+    unsigned int *err;               // device-side precondition counter (woden_check)
 };
 
 template <int FT, bool GAUSS>
@@ -90,6 +91,14 @@ predict_pg_kernel(const PGParams<typename std::conditional<GAUSS, GeoG, GeoP>::t
         for (int j = 0; j < FT; ++j) ns2[j] = p.chan_ns2[ftile * FT + j];
     }
     (void)ns2;
+    {
+        // the MAGIC23 hand-off holds while |phase| < 2^28 turns; |D nu/c| <= sqrt(2) |b| max(nu)/c
+        double smax = 0.0;
+#pragma unroll
+        for (int j = 0; j < FT; ++j) smax = fmax(smax, sf[j]);
+        const double bound = sqrt(fma(u, u, fma(v, v, w * w))) * 1.4142135623730951 * smax;
+        if (valid && !(bound < 268435456.0)) atomicAdd(p.err, 1u);
+    }
 
     float acc_re[FT], acc_im[FT];
 #pragma unroll
@@ -110,7 +119,7 @@ predict_pg_kernel(const PGParams<typename std::conditional<GAUSS, GeoG, GeoP>::t
                 const GeoG &gg = *reinterpret_cast<const GeoG *>(&g[k]);
                 const float gx = fmaf(gg.as, uf, gg.ac * vf);
                 const float gy = fmaf(gg.bc, uf, -gg.bs * vf);
-                Q = fmaf(gx, gx, gy * gy);
+                Q = fminf(fmaf(gx, gx, gy * gy), 1.0e30f);
             }
             (void)Q;
             float S[FT];
@@ -159,14 +168,14 @@ predict_pg_kernel(const PGParams<typename std::conditional<GAUSS, GeoG, GeoP>::t
 
 template <bool GAUSS, typename Geo>
 cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const float *flux, int n_pad,
-                   float2 *vis, int accumulate, cudaStream_t st)
+                   float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
     constexpr int FT = PG_FT;
     PGParams<Geo> p;
     p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m;
     p.geo = geo; p.flux = flux; p.chan_s = ch.s; p.chan_ns2 = ch.ns2; p.vis = vis;
     p.n_bt = (long long)uvw.T * uvw.B;
-    p.B = uvw.B; p.F = uvw.F; p.n_pad = n_pad; p.accumulate = accumulate;
+    p.B = uvw.B; p.F = uvw.F; p.n_pad = n_pad; p.accumulate = accumulate; p.err = err;
     const int smem = NSTAGE * KB * ((int)sizeof(Geo) + FT * 4);
     auto kern = predict_pg_kernel<FT, GAUSS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -179,15 +188,15 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const
 }  // namespace
 
 cudaError_t launch_predict_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st)
+                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
-    return launch<false>(uvw, ch, geo, flux, n_pad, vis, accumulate, st);
+    return launch<false>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
 }
 
 cudaError_t launch_predict_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
-                                     int n_pad, float2 *vis, int accumulate, cudaStream_t st)
+                                     int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
-    return launch<true>(uvw, ch, geo, flux, n_pad, vis, accumulate, st);
+    return launch<true>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
 }
 
 }  // namespace woden

@@ -55,6 +55,7 @@ struct WParams {
     long long n_bt;                  // T * B
     int B, F, n_pad, accumulate;
     double ds;                       // channel step / c
+    unsigned int *err;               // device-side precondition counter (woden_check)
 };
 
 // sign pattern of the recurrence: s_j = +1 for (j - J0) mod 4 in {0, 1}, else -1
@@ -69,14 +70,16 @@ struct Seed {
 
 template <bool GAUSS, typename Geo>
 __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, double w, float uf, float vf,
-                                          double sfA, double ds, Seed<GAUSS> &sd)
+                                          double sfA, double ds, double magic, int kshift, Seed<GAUSS> &sd)
 {
     // S3: D = u l + v m + w (n-1), FP64 metres
     const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
-    // frac(phase) as signed Q0.32 (low word of phase + 1.5*2^20): chain A's seed and the channel
+    // frac(phase) as signed Q0.32: the low word of phase + 1.5*2^(20+k) holds the phase modulo 2^k
+    // turns in units of 2^(k-32) turn, so a left shift by k leaves the fraction (k = 0 while the
+    // thread's phases stay below 2^19 turns; see phase_shift_for).  Chain A's seed and the channel
     // step by one DFMA each; chain B's seed, WH channels up, by integer arithmetic (wraps mod 1 turn)
-    const unsigned qA = (unsigned)__double2loint(fma(D, sfA, MAGIC32));
-    const unsigned qd = (unsigned)__double2loint(fma(D, ds, MAGIC32));
+    const unsigned qA = (unsigned)__double2loint(fma(D, sfA, magic)) << kshift;
+    const unsigned qd = (unsigned)__double2loint(fma(D, ds, magic)) << kshift;
     const unsigned qB = qA + (unsigned)WH * qd;
     const float thA = (float)(int)qA * Q32_TO_RAD;
     const float thB = (float)(int)qB * Q32_TO_RAD;
@@ -88,7 +91,7 @@ __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, doub
         // Eq 13-14 in metres: gx = cg maj (sin pa u + cos pa v), gy = cg min (cos pa u - sin pa v)
         const float gx = fmaf(g.as, uf, g.ac * vf);
         const float gy = fmaf(g.bc, uf, -g.bs * vf);
-        sd.Q = fmaf(gx, gx, gy * gy);
+        sd.Q = fminf(fmaf(gx, gx, gy * gy), 1.0e30f);     // finite: 0 x inf cannot arise below
     } else {
         sd.Q = 0.f;
     }
@@ -149,6 +152,14 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
     const double sfA = p.chan_s[ftile * FT + J0];
     const double sfB = p.chan_s[ftile * FT + H + J0];
     const double ds = p.ds;
+    // phase range of this thread: |D nu/c| <= sqrt(2) |b| max(nu)/c turns (l^2 + m^2 < 1)
+    const double smax = fmax(fabs(p.chan_s[ftile * FT]), fabs(p.chan_s[ftile * FT + FT - 1]));
+    int kshift = phase_shift_for(sqrt(fma(u, u, fma(v, v, w * w))) * 1.4142135623730951 * smax);
+    if (kshift > PHASE_MAX_SHIFT) {              // beyond 2^28 turns: counted for woden_check
+        if (valid) atomicAdd(p.err, 1u);
+        kshift = PHASE_MAX_SHIFT;
+    }
+    const double magic = magic32_shifted(kshift);
 
     EnvConst ec;
     ec.e0 = ec.ef = ec.eb = 0ull; ec.e2 = 0.f;
@@ -178,12 +189,12 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
         const unsigned char *fl = smem + s * STAGE_BYTES + GEO_BYTES;
 
         Seed<GAUSS> sd;
-        make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, ds, sd);
+        make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, ds, magic, kshift, sd);
 #pragma unroll (GAUSS ? 2 : 1)
         for (int k = 0; k < KB; ++k) {
             // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
             Seed<GAUSS> nx;
-            make_seed<GAUSS>(g[k + 1 < KB ? k + 1 : k], u, v, w, uf, vf, sfA, ds, nx);
+            make_seed<GAUSS>(g[k + 1 < KB ? k + 1 : k], u, v, w, uf, vf, sfA, ds, magic, kshift, nx);
 
             const ulonglong2 *fl2 = reinterpret_cast<const ulonglong2 *>(fl + (size_t)k * FT * 4);
             const float cf = sd.wr + sd.wr;                    // c = 2 cos(delta)
@@ -200,10 +211,15 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
                 const f32x2 Q2 = pack2(sd.Q, sd.Q);
                 unpack2(mul2(Q2, ec.e0), a, b);
                 xb = pack2(ex2_approx(a), ex2_approx(b));                 // xi at J0
+                // The step ratios are clamped to finite values: where xi at J0 has flushed to zero
+                // (Q s^2 > 126) a ratio 2^(+big) would give 0 x inf = NaN; clamped, the chain is an
+                // exact 0, which it is to 2^-90 because the walking path is only taken when a chain
+                // spans at most +-12.5 % in frequency (api.cu).  Where xi at J0 is normal the ratio
+                // exponents are <= 2 x 126 x 1/64 and the clamp is idle.
                 unpack2(mul2(Q2, ec.ef), a, b);
-                rf = pack2(ex2_approx(a), ex2_approx(b));                 // xi_{J0+1} / xi_{J0}
+                rf = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b, 126.f)));   // xi_{J0+1} / xi_{J0}
                 unpack2(mul2(Q2, ec.eb), a, b);
-                rb = pack2(ex2_approx(a), ex2_approx(b));                 // xi_{J0-1} / xi_{J0}
+                rb = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b, 126.f)));   // xi_{J0-1} / xi_{J0}
                 const float qf = ex2_approx(sd.Q * ec.e2);
                 qq = pack2(qf, qf);
                 xf = mul2(xb, rf);                                        // xi at J0 + 1
@@ -286,13 +302,13 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
 
 template <bool GAUSS, typename Geo>
 cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const float *flux, int n_pad,
-                   float2 *vis, int accumulate, cudaStream_t st)
+                   float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
     WParams<Geo> p;
     p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m;
     p.geo = geo; p.flux = flux; p.chan_s = ch.s; p.vis = vis;
     p.n_bt = (long long)uvw.T * uvw.B;
-    p.B = uvw.B; p.F = uvw.F; p.n_pad = n_pad; p.accumulate = accumulate; p.ds = ch.ds;
+    p.B = uvw.B; p.F = uvw.F; p.n_pad = n_pad; p.accumulate = accumulate; p.ds = ch.ds; p.err = err;
     const int smem = WSTAGES * KB * ((int)sizeof(Geo) + WALK_FT * 4);
     auto kern = predict_walk_kernel<GAUSS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -305,15 +321,15 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const
 }  // namespace
 
 cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                               int n_pad, float2 *vis, int accumulate, cudaStream_t st)
+                               int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
-    return launch<false>(uvw, ch, geo, flux, n_pad, vis, accumulate, st);
+    return launch<false>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
 }
 
 cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, cudaStream_t st)
+                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
 {
-    return launch<true>(uvw, ch, geo, flux, n_pad, vis, accumulate, st);
+    return launch<true>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
 }
 
 }  // namespace woden

@@ -34,11 +34,15 @@ def test_library_builds_and_exports_every_declared_symbol():
 def test_status_strings_and_constants_match_header():
     L = binding.load()
     src = open(HEADER).read()
+    pipes = {}
     for name, val in re.findall(r"#define\s+(WODEN_[A-Z_0-9]+)\s+(-?\d+)", src):
-        if name.startswith("WODEN_PIPE_"):
-            assert binding.PIPES[name[len("WODEN_PIPE_"):]] == int(val), name
+        if name == "WODEN_PIPE_COUNT":
+            assert len(binding.PIPES) == int(val)
+        elif name.startswith("WODEN_PIPE_"):
+            pipes[name[len("WODEN_PIPE_"):]] = int(val)
         else:
             assert getattr(binding, name) == int(val), name
+    assert pipes == binding.PIPES          # every pattern bench.py uses is a documented id
     for code in (0, -1, -2, -3, -4, -5, -6):
         assert L.woden_strerror(code).decode() not in ("", "unknown status")
     assert L.woden_strerror(-99).decode() == "unknown status"

@@ -457,3 +457,183 @@ def test_error_codes_and_device_side_checks(ctx, torch_mod):
     ctx.predict_shapelets(dw.uvw, sl, sm, ss0, sal, wl.ref_freq_hz, b1, b2, pa, M, off, nc, 3, n1, n2, cf, vis)
     with pytest.raises(binding.WodenError):
         ctx.check()
+
+
+# ---------------------------------------------------------------------------------------------
+# Round-2 edge cases of the point / Gaussian kernels: strongly resolved Gaussians, long baselines,
+# and the channel lists that may (not) take the channel-walking path.
+
+def _array_case(radius_m, T, B, F, f0_hz, step_hz, seed):
+    rng = np.random.default_rng(seed)
+    east, north = inputs.disk_antennas(rng, 40, radius_m)
+    u, v, w = inputs.uvw_metres(east, north, T, 8.0)
+    order = np.argsort(-(u[0] ** 2 + v[0] ** 2))            # keep the LONGEST baselines and a few short ones
+    keep = np.concatenate([order[: B - 20], order[-20:]])
+    u, v, w = (np.ascontiguousarray(a[:, keep]) for a in (u, v, w))
+    return u, v, w, f0_hz + step_hz * np.arange(F)
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
+@pytest.mark.parametrize("radius_m", [1500.0, 2750.0], ids=["3km", "5.5km"])
+@pytest.mark.parametrize("step_hz", [80e3, -80e3, 1.28e6, -1.28e6])
+def test_wide_gaussians_on_long_baselines_are_finite_and_match(ctx, torch_mod, path, radius_m, step_hz):
+    # Eq 12-14 with maj >= 0 as the header allows: FWHM from 0.5 to 20 degrees on
+    # 3 km / 5.5 km arrays.  The envelope underflows to an exact 0 on the long baselines (the oracle's
+    # exp() does the same); the channel-walking envelope recurrence must give 0 there, not 0 x inf.
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(path)
+    F = 40
+    f0 = 167e6 if step_hz > 0 else 200e6
+    u, v, w, fr = _array_case(radius_m, 2, 150, F, f0, step_hz, seed=int(radius_m))
+    rng = np.random.default_rng(99)
+    fwhm_deg = np.repeat([0.5, 1.5, 3.0, 6.0, 20.0], 4)
+    n = len(fwhm_deg)
+    maj = np.deg2rad(fwhm_deg)
+    mnr = maj * np.tile([1.0, 0.5, 0.05, 0.0], 5)
+    pa = rng.uniform(0, np.pi, n)
+    l, m = inputs.disk_lm(rng, n, 10.0)
+    s0 = inputs.log_uniform(rng, n, 0.5, 5.0) * rng.choice([-1.0, 1.0], n)
+    al = rng.normal(-0.8, 0.2, n)
+    uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+    d = lambda a: _dev(torch, a)
+    worst = 0.0
+    # each width class alone (a NaN or a wrong zero cannot hide behind other components), then all
+    for sel in [np.arange(4 * i, 4 * i + 4) for i in range(5)] + [np.arange(n)]:
+        vis = ctx.new_vis(uvw)
+        ctx.predict_gaussians(uvw, d(l[sel]), d(m[sel]), d(s0[sel]), d(al[sel]), 150e6, d(maj[sel]), d(mnr[sel]),
+                              d(pa[sel]), vis)
+        torch.cuda.synchronize(); ctx.check()
+        assert ctx.last_path() == (binding.WODEN_PATH_WALKING if path == 0 else binding.WODEN_PATH_GENERAL)
+        V = vis.cpu().numpy()
+        assert np.all(np.isfinite(V.view(np.float32)))
+        ref = oracle.predict_gaussians(u, v, w, fr, l[sel], m[sel], s0[sel], al[sel], 150e6, maj[sel], mnr[sel], pa[sel])
+        scale = oracle.tolerance_scale(fr, s0[sel], al[sel], 150e6)
+        worst = max(worst, float((np.abs(V - ref) / scale[None, :, None]).max()))
+    assert worst <= TOL
+    # the case is what it claims: some envelopes are an exact zero, some visibilities are not
+    assert np.abs(ref).min() < 1e-3 * np.abs(ref).max() and np.abs(ref).max() > 0.1
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
+def test_envelope_near_the_underflow_threshold(ctx, torch_mod, path):
+    # exponents Q s^2 swept through the FP32 flush threshold (2^-126) along the baseline axis: the
+    # walking envelope's seed flushes while neighbouring channels are still (barely) normal
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(path)
+    B, F = 400, 64
+    fr = 150e6 + 1.0e6 * np.arange(F)
+    u = np.linspace(50.0, 4000.0, B)[None, :].copy()
+    v = np.zeros((1, B)); w = np.zeros((1, B))
+    z = np.array([0.0])
+    maj = np.array([np.deg2rad(0.25)])
+    uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+    vis = ctx.new_vis(uvw)
+    ctx.predict_gaussians(uvw, _dev(torch, z), _dev(torch, z), _dev(torch, [1.0]), _dev(torch, z), 150e6,
+                          _dev(torch, maj), _dev(torch, maj), _dev(torch, z), vis)
+    torch.cuda.synchronize(); ctx.check()
+    V = vis.cpu().numpy()
+    ref = oracle.predict_gaussians(u, v, w, fr, z, z, [1.0], z, 150e6, maj, maj, z)
+    assert np.all(np.isfinite(V.view(np.float32)))
+    assert np.abs(V - ref).max() <= TOL
+    assert ref.real.min() < 1e-40 and ref.real.max() > 0.9          # spans the whole dynamic range
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
+@pytest.mark.parametrize("scale,f0", [(1.0e3, 180e6), (30.0, 10.0e9), (1.2e4, 1.4e9)],
+                         ids=["3000km@180MHz", "90km@10GHz", "36000km@1.4GHz"])
+def test_phase_hand_off_on_very_long_baselines(ctx, torch_mod, path, scale, f0):
+    # up to ~2^28 wavelengths: 5e5 ... 2e8 turns of phase.  The Q0.32 hand-off of the walking path
+    # shifts its fixed point per thread (phase.cuh); MAGIC23 of the general path holds to 2^28.
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(path)
+    u, v, w, fr = _array_case(1500.0, 2, 140, 37, f0, 80e3, seed=5)
+    u, v, w = u * scale, v * scale, w * scale
+    rng = np.random.default_rng(6)
+    n = 30
+    l, m = inputs.disk_lm(rng, n, 30.0)
+    s0 = inputs.log_uniform(rng, n, 0.1, 10.0)
+    al = rng.normal(-0.8, 0.2, n)
+    uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+    vis = ctx.new_vis(uvw)
+    ctx.predict_points(uvw, _dev(torch, l), _dev(torch, m), _dev(torch, s0), _dev(torch, al), 150e6, vis)
+    torch.cuda.synchronize(); ctx.check()
+    assert ctx.last_path() == (binding.WODEN_PATH_WALKING if path == 0 else binding.WODEN_PATH_GENERAL)
+    wavelengths = np.sqrt(u * u + v * v + w * w).max() * fr.max() / inputs.C_LIGHT
+    assert 2.0 ** 19 < wavelengths * 0.5 and np.sqrt(2.0) * wavelengths < 2.0 ** 28
+    ref = oracle.predict_points(u, v, w, fr, l, m, s0, al, 150e6)
+    sc = oracle.tolerance_scale(fr, s0, al, 150e6)
+    assert (np.abs(vis.cpu().numpy() - ref) / sc[None, :, None]).max() <= TOL
+
+
+@pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
+def test_baselines_beyond_the_phase_range_are_reported(ctx, torch_mod, path):
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(path)
+    u, v, w, fr = _array_case(1500.0, 1, 64, 16, 180e6, 80e3, seed=5)
+    u = u * 4.0e5                                          # ~1e9 m at 180 MHz: > 2^28 wavelengths
+    uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+    vis = ctx.new_vis(uvw)
+    ctx.check()
+    ctx.predict_points(uvw, _dev(torch, [0.01]), _dev(torch, [0.02]), _dev(torch, [1.0]), _dev(torch, [0.0]), 150e6, vis)
+    with pytest.raises(binding.WodenError) as e:
+        ctx.check()
+    assert e.value.status == binding.WODEN_ERR_DATA
+    ctx.check()
+
+
+def test_which_channel_lists_take_the_walking_path(ctx, torch_mod):
+    # woden_b200.h, woden_set_path: an arithmetic progression of >= 8 channels with step <= 1/64 of
+    # the lowest (padded) frequency walks; everything else is the general path.  The advisor's case:
+    # [100, 150, 200] MHz and a Gaussian whose envelope is 2^-7 at 100 MHz must not come out as 0.
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(0)
+    z = np.array([0.0])
+    cases = [
+        (167e6 + 80e3 * np.arange(16), True),
+        (167e6 + 80e3 * np.arange(8), True),
+        (167e6 + 80e3 * np.arange(7), False),                    # too short
+        (np.array([100e6, 150e6, 200e6]), False),
+        (100e6 + 50e6 * np.arange(9), False),                    # uniform but far too wide
+        (200e6 - 1.28e6 * np.arange(40), True),
+        (200e6 - 3.0e6 * np.arange(40), False),                  # continuation to 64 channels is too low
+        (167e6 + 80e3 * np.arange(16) ** 1.01, False),           # not equally spaced
+    ]
+    cg = np.pi / (2.0 * np.log(2.0))
+    for fr, walks in cases:
+        s_lo = fr.min() / inputs.C_LIGHT
+        ub = np.array([[30.0, 400.0, 2500.0]])
+        # circular Gaussian with envelope exactly 2^-7 on the 400 m baseline at the lowest frequency
+        maj = np.array([np.sqrt(7.0) / (cg * 400.0 * s_lo)])
+        uvw = binding.Uvw(_dev(torch, ub), _dev(torch, 0 * ub), _dev(torch, 0 * ub), fr)
+        vis = ctx.new_vis(uvw)
+        ctx.predict_gaussians(uvw, _dev(torch, z), _dev(torch, z), _dev(torch, [1.0]), _dev(torch, z), 150e6,
+                              _dev(torch, maj), _dev(torch, maj), _dev(torch, z), vis)
+        torch.cuda.synchronize(); ctx.check()
+        assert (ctx.last_path() == binding.WODEN_PATH_WALKING) == walks, fr[:3]
+        ref = oracle.predict_gaussians(ub, 0 * ub, 0 * ub, fr, z, z, [1.0], z, 150e6, maj, maj, z)
+        V = vis.cpu().numpy()
+        assert np.abs(V - ref).max() <= TOL
+        f_lo = int(np.argmin(fr))
+        assert abs(ref[0, f_lo, 1].real - 2.0 ** -7) < 1e-9 and abs(V[0, f_lo, 1].real - 2.0 ** -7) < 1e-6
+
+
+def test_non_finite_flux_at_any_channel_is_reported(ctx, torch_mod):
+    # s0 (nu/ref)^alpha overflows FP32 only at the upper channels: still counted (woden_check)
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(0)
+    u, v, w, _ = _small_case(seed=1, T=1, B=64, F=16)
+    fr = 150e6 * (1.0 + 0.01 * np.arange(1, 17))
+    uvw = binding.Uvw(_dev(torch, u), _dev(torch, v), _dev(torch, w), fr)
+    vis = ctx.new_vis(uvw)
+    al = np.array([np.log(3.0e38) / np.log(fr[8] / 150e6)])       # S(nu_8) ~ 3e38, S(nu_9 ...) > FLT_MAX
+    ctx.check()
+    ctx.predict_points(uvw, _dev(torch, [0.0]), _dev(torch, [0.0]), _dev(torch, [1.0]), _dev(torch, al), 150e6, vis)
+    with pytest.raises(binding.WodenError) as e:
+        ctx.check()
+    assert e.value.status == binding.WODEN_ERR_DATA
