@@ -254,7 +254,9 @@ int woden_shapelet_series(woden_ctx *ctx, int method, int p_max, long long n, co
 #define WODEN_PIPE_FFMA_3REG   10   /* FFMA with three distinct, changing register operands          */
 #define WODEN_PIPE_FFMA2_3REG  11   /* FFMA2 with three distinct, changing register pairs            */
 #define WODEN_PIPE_FFMA2_BCAST 12   /* FFMA2 with one fixed pair and two changing pairs              */
-#define WODEN_PIPE_COUNT       13
+#define WODEN_PIPE_FFMA2_UR    13   /* FFMA2 with two changing pairs and one uniform-register pair   */
+#define WODEN_PIPE_WALK        14   /* the channel-walking kernel's 4-FFMA2 pattern per channel pair */
+#define WODEN_PIPE_COUNT       15
 int woden_pipe_rate(woden_ctx *ctx, int which, int iters, double *thread_ops_per_s,
                     double *sm_clock_hz);
 

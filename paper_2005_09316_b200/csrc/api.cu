@@ -39,11 +39,14 @@ struct woden_ctx {
     int last_path = WODEN_PATH_NONE;
     cudaStream_t last_stream = nullptr;
     std::string last_error;
-    DevBuf geo, flux, tri, chan, err, hang, bmat, bscale, lut;
+    DevBuf geo, flux, tri, chan, err, hang, bmat, bscale, lut, wblocks;
     int lut_pm = -1, lut_nx = 0;
     double lut_dx = 0.0;
     int shapelet_path = WODEN_SHAPELET_AUTO;
     std::vector<double> chan_freqs;      // frequencies the device channel table was built from
+    std::vector<double> chan_s_host;     // nu_f / c of the padded channel list (host copy)
+    cudaStream_t walk_stream = nullptr;  // second lane of the channel-walking launches
+    cudaEvent_t walk_fork = nullptr, walk_join = nullptr;
     int chan_F_pad = 0;
     ChanTable ch{};
     // woden_simulate_host staging
@@ -136,6 +139,8 @@ int ensure_chan(woden_ctx *ctx, const woden_uvw *uvw, cudaStream_t st)
     CU(ctx, cudaMemcpyAsync(ctx->chan.p, host.data(), bytes, cudaMemcpyHostToDevice, st), "upload channel table");
     ctx->chan_freqs.assign(uvw->freqs_hz, uvw->freqs_hz + F);
     ctx->chan_F_pad = F_pad;
+    ctx->chan_s_host.assign(s, s + F_pad);
+    ctx->ch.s_host = ctx->chan_s_host.data();
     ctx->ch.s = reinterpret_cast<const double *>(ctx->chan.p);
     ctx->ch.nu = ctx->ch.s + F_pad;
     ctx->ch.ns2 = reinterpret_cast<const float *>(ctx->ch.nu + F_pad);
@@ -143,6 +148,15 @@ int ensure_chan(woden_ctx *ctx, const woden_uvw *uvw, cudaStream_t st)
     ctx->ch.F_pad = F_pad;
     ctx->ch.uniform = uniform;
     ctx->ch.ds = ds;
+    return WODEN_OK;
+}
+
+int ensure_walk_streams(woden_ctx *ctx)
+{
+    if (ctx->walk_stream) return WODEN_OK;
+    CU(ctx, cudaStreamCreateWithFlags(&ctx->walk_stream, cudaStreamNonBlocking), "create walk stream");
+    CU(ctx, cudaEventCreateWithFlags(&ctx->walk_fork, cudaEventDisableTiming), "create event");
+    CU(ctx, cudaEventCreateWithFlags(&ctx->walk_join, cudaEventDisableTiming), "create event");
     return WODEN_OK;
 }
 
@@ -209,11 +223,16 @@ int woden_destroy(woden_ctx *ctx)
     {
         Bind bind(ctx);
         cudaDeviceSynchronize();
+        if (ctx->walk_stream) {
+            cudaStreamDestroy(ctx->walk_stream);
+            cudaEventDestroy(ctx->walk_fork);
+            cudaEventDestroy(ctx->walk_join);
+        }
         if (ctx->copy_stream) {
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
         }
-        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->lut, &ctx->h_uvw, &ctx->h_comp,
+        for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->lut, &ctx->wblocks, &ctx->h_uvw, &ctx->h_comp,
                           &ctx->h_int, &ctx->h_vis})
             b->release();
     }
@@ -286,20 +305,27 @@ int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const doub
     const int n_pad = (n + KB - 1) / KB * KB;
     const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
     ctx->last_path = walk ? WODEN_PATH_WALKING : WODEN_PATH_GENERAL;
-    const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoP)), "alloc geometry");
-    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
     unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
     launch_pack_points(l, m, n, n_pad, static_cast<GeoP *>(ctx->geo.p), err, st);
-    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, FT, walk, static_cast<float *>(ctx->flux.p), err,
-                     st);
-    CU(ctx, cudaGetLastError(), "pack points");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
     const GeoP *geo = static_cast<const GeoP *>(ctx->geo.p);
-    const float *flux = static_cast<const float *>(ctx->flux.p);
     float2 *out = reinterpret_cast<float2 *>(vis);
-    CU(ctx, walk ? launch_walk_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st)
-                 : launch_predict_points(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st),
+    if (walk) {
+        if ((rc = ensure_walk_streams(ctx)) != WODEN_OK) return rc;
+        CU(ctx, ctx->wblocks.reserve(walk_blocks_bytes(n, ctx->ch.F_pad / WALK_FT, false)), "alloc constant blocks");
+        unsigned char *blocks = static_cast<unsigned char *>(ctx->wblocks.p);
+        launch_pack_walk_points(geo, s0_jy, alpha, ref_freq_hz, n, ctx->ch, blocks, err, st);
+        CU(ctx, cudaGetLastError(), "pack points");
+        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join};
+        CU(ctx, launch_walk_points(d, ctx->ch, blocks, n, out, accumulate ? 1 : 0, err, ws), "predict_points launch");
+        return WODEN_OK;
+    }
+    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, false, static_cast<float *>(ctx->flux.p), err, st);
+    CU(ctx, cudaGetLastError(), "pack points");
+    CU(ctx, launch_predict_points(d, ctx->ch, geo, static_cast<const float *>(ctx->flux.p), n_pad, out,
+                                  accumulate ? 1 : 0, err, st),
        "predict_points launch");
     return WODEN_OK;
 }
@@ -323,21 +349,29 @@ int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     const int n_pad = (n + KB - 1) / KB * KB;
     const bool walk = ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform;
     ctx->last_path = walk ? WODEN_PATH_WALKING : WODEN_PATH_GENERAL;
-    const int FT = walk ? WALK_FT : PG_FT;
     CU(ctx, ctx->geo.reserve((size_t)n_pad * sizeof(GeoG)), "alloc geometry");
-    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
     unsigned int *err = static_cast<unsigned int *>(ctx->err.p);
     launch_pack_gaussians(l, m, maj_fwhm_rad, min_fwhm_rad, pa_rad, n, n_pad, static_cast<GeoG *>(ctx->geo.p), err,
                           st);
-    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, FT, walk, static_cast<float *>(ctx->flux.p), err,
-                     st);
-    CU(ctx, cudaGetLastError(), "pack gaussians");
     UvwDev d{uvw->u_m, uvw->v_m, uvw->w_m, uvw->n_baselines, uvw->n_times, uvw->n_freqs};
     const GeoG *geo = static_cast<const GeoG *>(ctx->geo.p);
-    const float *flux = static_cast<const float *>(ctx->flux.p);
     float2 *out = reinterpret_cast<float2 *>(vis);
-    CU(ctx, walk ? launch_walk_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st)
-                 : launch_predict_gaussians(d, ctx->ch, geo, flux, n_pad, out, accumulate ? 1 : 0, err, st),
+    if (walk) {
+        if ((rc = ensure_walk_streams(ctx)) != WODEN_OK) return rc;
+        CU(ctx, ctx->wblocks.reserve(walk_blocks_bytes(n, ctx->ch.F_pad / WALK_FT, true)), "alloc constant blocks");
+        unsigned char *blocks = static_cast<unsigned char *>(ctx->wblocks.p);
+        launch_pack_walk_gaussians(geo, s0_jy, alpha, ref_freq_hz, n, ctx->ch, blocks, err, st);
+        CU(ctx, cudaGetLastError(), "pack gaussians");
+        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join};
+        CU(ctx, launch_walk_gaussians(d, ctx->ch, blocks, n, out, accumulate ? 1 : 0, err, ws),
+           "predict_gaussians launch");
+        return WODEN_OK;
+    }
+    CU(ctx, ctx->flux.reserve((size_t)ctx->ch.F_pad * n_pad * 4), "alloc flux table");
+    launch_pack_flux(s0_jy, alpha, ref_freq_hz, n, n_pad, ctx->ch, PG_FT, false, static_cast<float *>(ctx->flux.p), err, st);
+    CU(ctx, cudaGetLastError(), "pack gaussians");
+    CU(ctx, launch_predict_gaussians(d, ctx->ch, geo, static_cast<const float *>(ctx->flux.p), n_pad, out,
+                                     accumulate ? 1 : 0, err, st),
        "predict_gaussians launch");
     return WODEN_OK;
 }

@@ -39,12 +39,27 @@ cudaError_t launch_predict_points(const UvwDev &uvw, const ChanTable &ch, const 
 cudaError_t launch_predict_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo,
                                      const float *flux, int n_pad, float2 *vis, int accumulate,
                                      unsigned int *err, cudaStream_t st);
-// channel-walking path (predict_walk.cu): equally spaced channels only
+// channel-walking path (predict_walk.cu): equally spaced channels only.  Component data reaches the
+// kernel through the constant bank, one block of WALK_CB_BYTES per launch (half of the 64 KB bank):
+// launch_pack_walk_* fills blocks[(ftile * n_chunks + chunk)] in device memory from the packed
+// geometry records, launch_walk_* copies block after block into the bank and launches.
 constexpr int WALK_FT = 32;      // channels per thread: two chains of 16
-cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                               int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st);
-cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st);
+constexpr int WALK_CB_BYTES = 32768;
+constexpr int WALK_KC_POINTS = WALK_CB_BYTES / (32 + WALK_FT * 4);     // 204 components per launch
+constexpr int WALK_KC_GAUSS = WALK_CB_BYTES / (48 + WALK_FT * 4);      // 186
+struct WalkStreams {
+    cudaStream_t main, aux;      // the caller's stream and the context's second lane
+    cudaEvent_t fork, join;
+};
+size_t walk_blocks_bytes(int n, int n_ftiles, bool gauss);
+void launch_pack_walk_points(const GeoP *geo, const double *s0, const double *alpha, double ref_freq, int n,
+                             const ChanTable &ch, unsigned char *blocks, unsigned int *err, cudaStream_t st);
+void launch_pack_walk_gaussians(const GeoG *geo, const double *s0, const double *alpha, double ref_freq, int n,
+                                const ChanTable &ch, unsigned char *blocks, unsigned int *err, cudaStream_t st);
+cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n,
+                               float2 *vis, int accumulate, unsigned int *err, const WalkStreams &ws);
+cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n,
+                                  float2 *vis, int accumulate, unsigned int *err, const WalkStreams &ws);
 
 constexpr int SH_FT = 1;         // flux table tile for shapelets: [F][n] layout
 int shapelet_order_bucket(int p_max);     // compile-time order PM >= p_max, or -1

@@ -57,6 +57,7 @@ __host__ __device__ constexpr int tri_stride(int PM) { return tri_size(PM) + ((t
 //   ns2[f]  = -(nu_f / c)^2       (FP32, Gaussian exponent scale)
 // padded with zeros to F_pad (a multiple of the channel tile).
 struct ChanTable {
+    const double *s_host;   // HOST copy of s[] (per-launch scalars of the channel-walking kernel)
     const double *s;
     const double *nu;
     const float *ns2;

@@ -17,7 +17,9 @@ constexpr int PIPE_CTAS_PER_SM = 2;
 
 enum { P_FFMA = 0, P_MUFU = 1, P_DFMA = 2, P_I2F = 3, P_LOP3 = 4, P_FFMA2 = 5, P_FFMA_IMM = 6,
        P_F2F = 7, P_MUFU_EX2 = 8, P_MUFU_FFMA = 9, P_FFMA_3REG = 10, P_FFMA2_3REG = 11, P_FFMA2_BCAST = 12,
-       P_COUNT };
+       P_FFMA2_UR = 13, P_WALK = 14, P_COUNT };
+
+__constant__ unsigned long long PIPE_C[1024];     // uniform operands (values are irrelevant: zero)
 
 __device__ __forceinline__ uint64_t globaltimer_ns()
 {
@@ -108,6 +110,61 @@ __global__ void __launch_bounds__(PIPE_THREADS) pipe_kernel(int iters, float see
                     asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i]), "=f"(a[i + 1]) : "l"(x));
                     asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i + 2]), "=f"(a[i + 3]) : "l"(y));
                 }
+        } else if (WHICH == P_FFMA2_UR) {
+            // x = fma2(y, U, x): two changing register pairs + one uniform-register pair (constant bank)
+            unsigned long long x[CHAINS / 4], y[CHAINS / 4];
+#pragma unroll
+            for (int i = 0; i < CHAINS / 4; ++i) {
+                asm("mov.b64 %0, {%1, %2};" : "=l"(x[i]) : "f"(a[4 * i]), "f"(a[4 * i + 1]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(y[i]) : "f"(a[4 * i + 2]), "f"(a[4 * i + 3]));
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int i = 0; i < CHAINS / 4; ++i) {
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(x[i]) : "l"(y[i]), "l"(PIPE_C[(it * 32 + r * 8 + 2 * i) & 1023]));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(y[i]) : "l"(x[i]), "l"(PIPE_C[(it * 32 + r * 8 + 2 * i + 1) & 1023]));
+                }
+#pragma unroll
+            for (int i = 0; i < CHAINS / 4; ++i) {
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[4 * i]), "=f"(a[4 * i + 1]) : "l"(x[i]));
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[4 * i + 2]), "=f"(a[4 * i + 3]) : "l"(y[i]));
+            }
+        } else if (WHICH == P_WALK) {
+            // the channel-walking kernel's instruction pattern per channel pair (predict_walk.cu), two
+            // independent chains: rn = c rc + ra; in = c ic + ia (scalar c); acc_re += U rc; acc_im += U ic
+            unsigned long long rc[2], ic[2], ra[2], ia[2], ar[2], ai[2], cc;
+            asm("mov.b64 %0, {%1, %2};" : "=l"(cc) : "f"(b), "f"(b));
+#pragma unroll
+            for (int d = 0; d < 2; ++d) {
+                asm("mov.b64 %0, {%1, %2};" : "=l"(rc[d]) : "f"(a[8 * d]), "f"(a[8 * d + 1]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(ic[d]) : "f"(a[8 * d + 2]), "f"(a[8 * d + 3]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(ra[d]) : "f"(a[8 * d + 4]), "f"(a[8 * d + 5]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(ia[d]) : "f"(a[8 * d + 6]), "f"(a[8 * d + 7]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(ar[d]) : "r"(u[8 * d]), "r"(u[8 * d + 1]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(ai[d]) : "r"(u[8 * d + 2]), "r"(u[8 * d + 3]));
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int d = 0; d < 2; ++d) {
+                    const unsigned long long U = PIPE_C[(it * 16 + r * 2 + d) & 1023];
+                    unsigned long long rn, in;
+                    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rn) : "l"(cc), "l"(rc[d]), "l"(ra[d]));
+                    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(in) : "l"(cc), "l"(ic[d]), "l"(ia[d]));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(ar[d]) : "l"(U), "l"(rc[d]));
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(ai[d]) : "l"(U), "l"(ic[d]));
+                    ra[d] = rc[d]; ia[d] = ic[d]; rc[d] = rn; ic[d] = in;
+                }
+#pragma unroll
+            for (int d = 0; d < 2; ++d) {
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[8 * d]), "=f"(a[8 * d + 1]) : "l"(rc[d]));
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[8 * d + 2]), "=f"(a[8 * d + 3]) : "l"(ic[d]));
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[8 * d + 4]), "=f"(a[8 * d + 5]) : "l"(ra[d]));
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(a[8 * d + 6]), "=f"(a[8 * d + 7]) : "l"(ia[d]));
+                asm("mov.b64 {%0, %1}, %2;" : "=r"(u[8 * d]), "=r"(u[8 * d + 1]) : "l"(ar[d]));
+                asm("mov.b64 {%0, %1}, %2;" : "=r"(u[8 * d + 2]), "=r"(u[8 * d + 3]) : "l"(ai[d]));
+            }
         } else if (WHICH == P_MUFU) {
 #pragma unroll
             for (int i = 0; i < CHAINS; i += 2) {
@@ -165,6 +222,8 @@ double ops_per_iter(int which)
     switch (which) {
     case P_FFMA: case P_FFMA_IMM: case P_LOP3: return 4.0 * CHAINS;
     case P_FFMA2: case P_FFMA2_3REG: case P_FFMA2_BCAST: return 4.0 * CHAINS;   // scalar FMAs (2 per f32x2)
+    case P_FFMA2_UR: return 4.0 * CHAINS;      // 4 x 8 FFMA2 = 64 scalar FMAs
+    case P_WALK: return 8.0 * 2 * 4 * 2;       // 8 steps x 2 chains x 4 FFMA2 x 2 lanes
     case P_FFMA_3REG: return 4.0 * CHAINS;
     case P_MUFU: case P_MUFU_EX2: case P_I2F: return CHAINS;
     case P_MUFU_FFMA: return CHAINS / 8 * 2;    // MUFU ops; 12 FFMA ride along per 2 MUFU
@@ -220,6 +279,8 @@ cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double
     case P_FFMA_3REG: err = run_one<P_FFMA_3REG>(iters, grid, sink, clk, &ms); break;
     case P_FFMA2_3REG: err = run_one<P_FFMA2_3REG>(iters, grid, sink, clk, &ms); break;
     case P_FFMA2_BCAST: err = run_one<P_FFMA2_BCAST>(iters, grid, sink, clk, &ms); break;
+    case P_FFMA2_UR: err = run_one<P_FFMA2_UR>(iters, grid, sink, clk, &ms); break;
+    case P_WALK: err = run_one<P_WALK>(iters, grid, sink, clk, &ms); break;
     }
     if (err == cudaSuccess) err = cudaMemcpy(hclk, clk, 16, cudaMemcpyDeviceToHost);
     cudaFree(sink); cudaFree(clk);

@@ -6,7 +6,8 @@
 // Mapping: one thread owns one (baseline, time) pair and WFT = 32 consecutive channels, held as
 // two chains of WH = 16 (channels j and j + 16) that ride in the two lanes of the packed FP32x2
 // instructions of sm_100 (SASS FFMA2 / FMUL2).  All 2 x 32 accumulators stay in registers for
-// the whole sum over components (no atomics; the paper's atomicAdd, is prior art).
+// the sum over the components of one launch (no atomics; the paper's atomicAdd, is
+// prior art).
 //
 // Per (thread, component):
 //   D = u_m l + v_m m + w_m (n-1)                       FP64 metres (3 FP64 ops, hard part H1)
@@ -26,35 +27,62 @@
 //   The kernel accumulates sum S q with q = exp(+i theta), theta = 2 pi frac(phi);
 //   exp(-2 pi i phi) = conj(q), so the epilogue stores (re, -im).
 //
-// Staging: component geometry (32 / 48 B) and the 32 precomputed fluxes S_k(nu_f) of the tile are
-// fetched in blocks of KB = 64 components by 1-D bulk async copies (TMA engine, SASS UBLKCP) into a
-// 4-stage ring with full/empty mbarriers: warps release a stage when done and only the producer
-// thread waits, so the warps of a CTA drift freely within two blocks (no __syncthreads in the loop).
+// Operand delivery.  The register file of an SM sub-partition feeds about
+// two 32-bit operands per lane per clock, so an FFMA2 with three fresh register pairs costs three
+// cycles instead of two (profiles/pipes_r1.txt).  Everything a component contributes besides the
+// thread's own baseline -- its direction (l, m, n-1), its envelope scales and its 32 fluxes
+// S_k(nu_f) of the channel tile -- is the same for every thread of the launch, so it is served from
+// the CONSTANT BANK: ptxas loads it into uniform registers (SASS LDCU) and the accumulate becomes
+// FFMA2 R, R, UR, R with two register pairs.  There is no shared-memory staging, no barrier and no
+// divergent branch in the kernel.  The price is that the constant bank is fixed per launch: one
+// launch covers one channel tile and one block of <= 204 (186) components (32 KB of the 64 KB
+// bank); the accumulators are carried from launch to launch through the output buffer (a
+// read-modify-write of 8 B per visibility per launch, < 10 % of the launch's duration on
+// HBM and overlapped by the other CTAs).  Launches alternate between the two halves of the bank
+// and between two streams that own disjoint parts of the output, so the copy into one half and the
+// tail of one launch hide behind the launch running from the other half.
 #include <type_traits>
 
 #include "kernels.h"
 #include "phase.cuh"
-#include "ptx.cuh"
 
 namespace woden {
 namespace {
 
+#ifndef WALK_THREADS
+#define WALK_THREADS 128
+#define WALK_CTAS 4
+#endif
+constexpr int WTHREADS = WALK_THREADS;   // (baseline, time) pairs per CTA
 constexpr int WH = WALK_FT / 2;      // chain length
 constexpr int WJ0 = WH / 2 - 1;      // seed position (and WJ0 + 1)
-constexpr int WSTAGES = 4;
-constexpr int WLAG = 2;              // the producer refills the stage consumed WLAG blocks ago
-constexpr int WWARPS = PG_THREADS / 32;
 
+// one launch's constants: per component its geometry record and 16 flux words (S[j], S[j + WH]),
+// interleaved so that every constant-bank offset in the loop body is a small immediate
 template <typename Geo>
+struct WalkRec {
+    Geo geo;
+    ulonglong2 flux[WH / 2];          // 128-bit granule q = words 2q, 2q + 1
+};
+template <typename Geo>
+struct WalkBlock {
+    static constexpr int KC = WALK_CB_BYTES / (int)sizeof(WalkRec<Geo>);
+    WalkRec<Geo> rec[KC];
+};
+static_assert(sizeof(WalkBlock<GeoP>) <= WALK_CB_BYTES && sizeof(WalkBlock<GeoG>) <= WALK_CB_BYTES, "constant block");
+static_assert(WalkBlock<GeoP>::KC == WALK_KC_POINTS && WalkBlock<GeoG>::KC == WALK_KC_GAUSS, "kernels.h constants");
+
+__constant__ __align__(16) unsigned char CBANK[2 * WALK_CB_BYTES];
+
 struct WParams {
     const double *u_m, *v_m, *w_m;   // [T][B]
-    const Geo *geo;                  // [n_pad]
-    const float *flux;               // [n_ftiles][n_pad][WALK_FT], chains interleaved
-    const double *chan_s;            // [F_pad], extrapolated past F
     float2 *vis;                     // [T][F][B]
-    long long n_bt;                  // T * B
-    int B, F, n_pad, accumulate;
-    double ds;                       // channel step / c
+    long long bt0, bt1;              // (baseline, time) pairs of this launch: [bt0, bt1)
+    int B, F, ftile;
+    int k0, n_k;                     // first record of this launch's block in the bank; components in it
+    int load_acc;                    // 1: continue from the values in vis, 0: start from zero
+    int first;                       // first block of the call: range violations are counted once
+    double sfA, sfB, ds, smax;       // nu/c at the two seed channels, channel step / c, max |nu/c| of the tile
     unsigned int *err;               // device-side precondition counter (woden_check)
 };
 
@@ -104,59 +132,27 @@ struct EnvConst {
 };
 
 template <bool GAUSS>
-__global__ void __launch_bounds__(PG_THREADS, 2)
-predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::type> p)
+__global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const WParams p)
 {
     using Geo = typename std::conditional<GAUSS, GeoG, GeoP>::type;
     constexpr int FT = WALK_FT, H = WH, J0 = WJ0;
-    constexpr int GEO_BYTES = KB * (int)sizeof(Geo);
-    constexpr int FLUX_BYTES = KB * FT * 4;
-    constexpr int STAGE_BYTES = GEO_BYTES + FLUX_BYTES;
+    // the bank as one array of records; k0 is a run-time value on purpose: the record index then
+    // carries the half's base and every constant-bank offset below is a small immediate
+    const WalkRec<Geo> *const rec = reinterpret_cast<const WalkRec<Geo> *>(CBANK);
+    const int k0 = p.k0, k1 = p.k0 + p.n_k;
 
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ __align__(8) uint64_t full_bar[WSTAGES];
-    __shared__ __align__(8) uint64_t empty_bar[WSTAGES];
-
-    const int tid = threadIdx.x;
-    const long long bt = (long long)blockIdx.x * PG_THREADS + tid;
-    const bool valid = bt < p.n_bt;
-    const int ftile = blockIdx.y;
-    const int n_blk = p.n_pad / KB;
-
-    const char *geo_src = reinterpret_cast<const char *>(p.geo);
-    const char *flux_src = reinterpret_cast<const char *>(p.flux + (size_t)ftile * p.n_pad * FT);
-
-    auto issue = [&](int blk) {
-        const int s = blk % WSTAGES;
-        mbar_arrive_expect_tx(&full_bar[s], STAGE_BYTES);
-        bulk_g2s(smem + s * STAGE_BYTES, geo_src + (size_t)blk * GEO_BYTES, GEO_BYTES, &full_bar[s]);
-        bulk_g2s(smem + s * STAGE_BYTES + GEO_BYTES, flux_src + (size_t)blk * FLUX_BYTES, FLUX_BYTES,
-                 &full_bar[s]);
-    };
-
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < WSTAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], WWARPS); }
-        fence_mbar_init();
-    }
-    __syncthreads();
-    if (tid == 0) {
-        const int pre = n_blk < WSTAGES ? n_blk : WSTAGES;
-        for (int b = 0; b < pre; ++b) issue(b);
-    }
+    const long long bt = p.bt0 + (long long)blockIdx.x * WTHREADS + threadIdx.x;
+    const bool valid = bt < p.bt1;
 
     // S1: this thread's baseline in metres; nu/c at the two chains' seed channels
     double u = 0.0, v = 0.0, w = 0.0;
     if (valid) { u = p.u_m[bt]; v = p.v_m[bt]; w = p.w_m[bt]; }
     const float uf = (float)u, vf = (float)v;
-    const double sfA = p.chan_s[ftile * FT + J0];
-    const double sfB = p.chan_s[ftile * FT + H + J0];
-    const double ds = p.ds;
+    const double sfA = p.sfA, sfB = p.sfB, ds = p.ds;
     // phase range of this thread: |D nu/c| <= sqrt(2) |b| max(nu)/c turns (l^2 + m^2 < 1)
-    const double smax = fmax(fabs(p.chan_s[ftile * FT]), fabs(p.chan_s[ftile * FT + FT - 1]));
-    int kshift = phase_shift_for(sqrt(fma(u, u, fma(v, v, w * w))) * 1.4142135623730951 * smax);
+    int kshift = phase_shift_for(sqrt(fma(u, u, fma(v, v, w * w))) * 1.4142135623730951 * p.smax);
     if (kshift > PHASE_MAX_SHIFT) {              // beyond 2^28 turns: counted for woden_check
-        if (valid) atomicAdd(p.err, 1u);
+        if (valid && p.first) atomicAdd(p.err, 1u);
         kshift = PHASE_MAX_SHIFT;
     }
     const double magic = magic32_shifted(kshift);
@@ -172,164 +168,234 @@ predict_walk_kernel(const WParams<typename std::conditional<GAUSS, GeoG, GeoP>::
         ec.e2 = (float)(-2.0 * ds * ds);
     }
 
+    // accumulators: y_j = s_j x_j of q = conj(exp(-2 pi i phi)); the output holds V = (s re, -s im),
+    // a transformation that is its own inverse, so a later launch reloads them the same way
+    const long long t = valid ? bt / p.B : 0;
+    const int b = valid ? (int)(bt - t * p.B) : 0;
+    float2 *const row = p.vis + ((size_t)t * p.F + (size_t)p.ftile * FT) * p.B + b;
     f32x2 acc_re[H], acc_im[H];
+    if (p.load_acc) {
 #pragma unroll
-    for (int j = 0; j < H; ++j) { acc_re[j] = 0ull; acc_im[j] = 0ull; }
-
-    for (int blk = 0; blk < n_blk; ++blk) {
-        const int s = blk % WSTAGES;
-        // producer: refill the stage every warp released WLAG blocks ago
-        if (tid == 0 && blk >= WLAG && blk - WLAG + WSTAGES < n_blk) {
-            const int ob = blk - WLAG;
-            mbar_wait(&empty_bar[ob % WSTAGES], (ob / WSTAGES) & 1);
-            issue(ob + WSTAGES);
+        for (int j = 0; j < H; ++j) {
+            float2 a = make_float2(0.f, 0.f), c = make_float2(0.f, 0.f);
+            if (valid && p.ftile * FT + j < p.F) a = row[(size_t)j * p.B];
+            if (valid && p.ftile * FT + j + H < p.F) c = row[(size_t)(j + H) * p.B];
+            const float sg = walk_neg(j) ? -1.f : 1.f;
+            acc_re[j] = pack2(sg * a.x, sg * c.x);
+            acc_im[j] = pack2(-sg * a.y, -sg * c.y);
         }
-        mbar_wait(&full_bar[s], (blk / WSTAGES) & 1);
-        const Geo *g = reinterpret_cast<const Geo *>(smem + s * STAGE_BYTES);
-        const unsigned char *fl = smem + s * STAGE_BYTES + GEO_BYTES;
-
-        Seed<GAUSS> sd;
-        make_seed<GAUSS>(g[0], u, v, w, uf, vf, sfA, ds, magic, kshift, sd);
-#pragma unroll (GAUSS ? 2 : 1)
-        for (int k = 0; k < KB; ++k) {
-            // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
-            Seed<GAUSS> nx;
-            make_seed<GAUSS>(g[k + 1 < KB ? k + 1 : k], u, v, w, uf, vf, sfA, ds, magic, kshift, nx);
-
-            const ulonglong2 *fl2 = reinterpret_cast<const ulonglong2 *>(fl + (size_t)k * FT * 4);
-            const float cf = sd.wr + sd.wr;                    // c = 2 cos(delta)
-            const f32x2 c2 = pack2(cf, cf), nc2 = pack2(-cf, -cf);
-            const f32x2 wr = pack2(sd.wr, sd.wr), wi = pack2(sd.wi, sd.wi), nwi = pack2(-sd.wi, -sd.wi);
-            // positions J0 (MUFU) and J0 + 1 (one complex rotation); s_J0 = s_{J0+1} = +1
-            const f32x2 r0 = pack2(sd.cA, sd.cB), i0 = pack2(sd.sA, sd.sB);
-            const f32x2 r1 = fma2(i0, nwi, mul2(r0, wr));
-            const f32x2 i1 = fma2(r0, wi, mul2(i0, wr));
-
-            f32x2 xf = 0ull, rf = 0ull, xb = 0ull, rb = 0ull, qq = 0ull;
-            if constexpr (GAUSS) {
-                float a, b;
-                const f32x2 Q2 = pack2(sd.Q, sd.Q);
-                unpack2(mul2(Q2, ec.e0), a, b);
-                xb = pack2(ex2_approx(a), ex2_approx(b));                 // xi at J0
-                // The step ratios are clamped to finite values: where xi at J0 has flushed to zero
-                // (Q s^2 > 126) a ratio 2^(+big) would give 0 x inf = NaN; clamped, the chain is an
-                // exact 0, which it is to 2^-90 because the walking path is only taken when a chain
-                // spans at most +-12.5 % in frequency (api.cu).  Where xi at J0 is normal the ratio
-                // exponents are <= 2 x 126 x 1/64 and the clamp is idle.
-                unpack2(mul2(Q2, ec.ef), a, b);
-                rf = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b, 126.f)));   // xi_{J0+1} / xi_{J0}
-                unpack2(mul2(Q2, ec.eb), a, b);
-                rb = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b, 126.f)));   // xi_{J0-1} / xi_{J0}
-                const float qf = ex2_approx(sd.Q * ec.e2);
-                qq = pack2(qf, qf);
-                xf = mul2(xb, rf);                                        // xi at J0 + 1
-                rf = mul2(rf, qq);                                        // ratio J0+1 -> J0+2
-            }
-
-            // flux words: 64-bit word j holds (S[j], S[j + H]); one LDS.128 = words 2q, 2q + 1.
-            // Each value is accumulated right AFTER the recurrence step that consumes it as its
-            // multiplicand, so both instructions read it in the same operand slot (register reuse
-            // cache: the register file delivers only two 32-bit operands per cycle, which makes an
-            // FFMA2 with three fresh register pairs cost 3 cycles instead of 2; profiles/pipes_r1.txt).
-            static_assert(J0 % 2 == 1, "seed position must be the high word of a 128-bit flux granule");
-            // ---- forward: y_{j+1} = (s_{j+1} s_j) c y_j + y_{j-1}; accumulates positions J0+1 .. H-1
-            {
-                f32x2 ra = r0, ia = i0, rc = r1, ic = i1, Skeep = 0ull;
+    } else {
 #pragma unroll
-                for (int j = J0 + 1; j < H; ++j) {
-                    f32x2 rn = 0ull, in = 0ull;
-                    if (j + 1 < H) {
-                        const f32x2 cc = (walk_neg(j + 1) != walk_neg(j)) ? nc2 : c2;
-                        rn = fma2(cc, rc, ra); in = fma2(cc, ic, ia);
-                    }
-                    f32x2 Sj;
-                    if (j % 2 == 1) { Sj = Skeep; }                            // high word of the granule in hand
-                    else { const ulonglong2 q = fl2[j / 2]; Sj = q.x; Skeep = q.y; }
-                    if constexpr (GAUSS) { Sj = mul2(Sj, xf); if (j + 1 < H) { xf = mul2(xf, rf); rf = mul2(rf, qq); } }
-                    acc_re[j] = fma2(Sj, rc, acc_re[j]);
-                    acc_im[j] = fma2(Sj, ic, acc_im[j]);
-                    ra = rc; ia = ic; rc = rn; ic = in;
-                }
-            }
-            // ---- backward: y_{j-1} = (s_{j-1} s_j) c y_j + y_{j+1}; accumulates positions J0 .. 0
-            {
-                f32x2 ra = r1, ia = i1, rc = r0, ic = i0, Skeep = 0ull;
-#pragma unroll
-                for (int j = J0; j >= 0; --j) {
-                    f32x2 rn = 0ull, in = 0ull;
-                    if (j >= 1) {
-                        const f32x2 cc = (walk_neg(j - 1) != walk_neg(j)) ? nc2 : c2;
-                        rn = fma2(cc, rc, ra); in = fma2(cc, ic, ia);
-                    }
-                    f32x2 Sj;
-                    if (j % 2 == 0) { Sj = Skeep; }                            // low word of the granule in hand
-                    else { const ulonglong2 q = fl2[j / 2]; Sj = q.y; Skeep = q.x; }
-                    if constexpr (GAUSS) { Sj = mul2(Sj, xb); if (j >= 1) { xb = mul2(xb, rb); rb = mul2(rb, qq); } }
-                    acc_re[j] = fma2(Sj, rc, acc_re[j]);
-                    acc_im[j] = fma2(Sj, ic, acc_im[j]);
-                    ra = rc; ia = ic; rc = rn; ic = in;
-                }
-            }
-            sd = nx;
-        }
-        // consumer release: this warp is done reading stage s
-        __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+        for (int j = 0; j < H; ++j) { acc_re[j] = 0ull; acc_im[j] = 0ull; }
     }
 
-    // S7: exp(-2 pi i phi) = conj(q): V = (re, -im); coalesced float2 stores along b
-    if (valid) {
-        const long long t = bt / p.B;
-        const int b = (int)(bt - t * p.B);
+    Seed<GAUSS> sd;
+    make_seed<GAUSS>(rec[k0].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, sd);
+#pragma unroll 2
+    for (int k = k0; k < k1; ++k) {
+        // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
+        Seed<GAUSS> nx;
+        make_seed<GAUSS>(rec[k + 1 < k1 ? k + 1 : k].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, nx);
+
+        // word j = (S[j], S[j + H]), read as 128-bit granules into uniform registers
+        const ulonglong2 *fl = rec[k].flux;
+        const float cf = sd.wr + sd.wr;                    // c = 2 cos(delta)
+        const f32x2 c2 = pack2(cf, cf), nc2 = pack2(-cf, -cf);
+        const f32x2 wr = pack2(sd.wr, sd.wr), wi = pack2(sd.wi, sd.wi), nwi = pack2(-sd.wi, -sd.wi);
+        // positions J0 (MUFU) and J0 + 1 (one complex rotation); s_J0 = s_{J0+1} = +1
+        const f32x2 r0 = pack2(sd.cA, sd.cB), i0 = pack2(sd.sA, sd.sB);
+        const f32x2 r1 = fma2(i0, nwi, mul2(r0, wr));
+        const f32x2 i1 = fma2(r0, wi, mul2(i0, wr));
+
+        f32x2 xf = 0ull, rf = 0ull, xb = 0ull, rb = 0ull, qq = 0ull;
+        if constexpr (GAUSS) {
+            float a, b2;
+            const f32x2 Q2 = pack2(sd.Q, sd.Q);
+            unpack2(mul2(Q2, ec.e0), a, b2);
+            xb = pack2(ex2_approx(a), ex2_approx(b2));                // xi at J0
+            // The step ratios are clamped to finite values: where xi at J0 has flushed to zero
+            // (Q s^2 > 126) a ratio 2^(+big) would give 0 x inf = NaN; clamped, the chain is an
+            // exact 0, which it is to 2^-90 because the walking path is only taken when a chain
+            // spans at most +-12.5 % in frequency (api.cu).  Where xi at J0 is normal the ratio
+            // exponents are <= 2 x 126 x 1/64 and the clamp is idle.
+            unpack2(mul2(Q2, ec.ef), a, b2);
+            rf = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b2, 126.f)));   // xi_{J0+1} / xi_{J0}
+            unpack2(mul2(Q2, ec.eb), a, b2);
+            rb = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b2, 126.f)));   // xi_{J0-1} / xi_{J0}
+            const float qf = ex2_approx(sd.Q * ec.e2);
+            qq = pack2(qf, qf);
+            xf = mul2(xb, rf);                                        // xi at J0 + 1
+            rf = mul2(rf, qq);                                        // ratio J0+1 -> J0+2
+        }
+
+        // ---- both directions in lock step: forward y_{j+1} = (s_{j+1} s_j) c y_j + y_{j-1} over positions
+        // J0+1 .. H-1, backward y_{j-1} = (s_{j-1} s_j) c y_j + y_{j+1} over J0 .. 0.  At step t the
+        // forward chain sits at jf = J0 + 1 + t and the backward chain at jb = J0 - t; the sign pattern is
+        // symmetric about J0 + 1/2, so the four recurrence FMAs of a step share one scalar (+c or -c):
+        // issued back to back they read it once (operand reuse), see DESIGN.md section 7.
+        {
+            f32x2 fra = r0, fia = i0, frc = r1, fic = i1;      // forward: previous, current
+            f32x2 bra = r1, bia = i1, brc = r0, bic = i0;      // backward
 #pragma unroll
-        for (int j = 0; j < FT; ++j) {
-            const int f = ftile * FT + j;
-            float a0, a1, b0, b1;
-            unpack2(acc_re[j % H], a0, a1);
-            unpack2(acc_im[j % H], b0, b1);
-            float re = j < H ? a0 : a1;
-            float im = j < H ? b0 : b1;
-            if (walk_neg(j % H)) { re = -re; im = -im; }      // s_j of the recurrence
-            if (f < p.F) {
-                float2 *dst = p.vis + ((size_t)t * p.F + f) * p.B + b;
-                float2 val = make_float2(re, -im);
-                if (p.accumulate) { const float2 old = *dst; val.x += old.x; val.y += old.y; }
-                *dst = val;
+            for (int t = 0; t < H / 2; ++t) {
+                const int jf = J0 + 1 + t, jb = J0 - t;
+                static_assert(H == 2 * (J0 + 1), "chains are walked symmetrically");
+                f32x2 frn = 0ull, fin = 0ull, brn = 0ull, bin = 0ull;
+                if (t + 1 < H / 2) {
+                    const bool flip = walk_neg(jf + 1) != walk_neg(jf);
+                    const f32x2 cc = flip ? nc2 : c2;           // same for jb - 1 vs jb (symmetry)
+                    frn = fma2(cc, frc, fra); fin = fma2(cc, fic, fia);
+                    brn = fma2(cc, brc, bra); bin = fma2(cc, bic, bia);
+                }
+                f32x2 Sf = (jf & 1) ? fl[jf >> 1].y : fl[jf >> 1].x;
+                f32x2 Sb = (jb & 1) ? fl[jb >> 1].y : fl[jb >> 1].x;
+                if constexpr (GAUSS) {
+                    Sf = mul2(Sf, xf); Sb = mul2(Sb, xb);
+                    if (t + 1 < H / 2) { xf = mul2(xf, rf); rf = mul2(rf, qq); xb = mul2(xb, rb); rb = mul2(rb, qq); }
+                }
+                acc_re[jf] = fma2(Sf, frc, acc_re[jf]);
+                acc_im[jf] = fma2(Sf, fic, acc_im[jf]);
+                acc_re[jb] = fma2(Sb, brc, acc_re[jb]);
+                acc_im[jb] = fma2(Sb, bic, acc_im[jb]);
+                fra = frc; fia = fic; frc = frn; fic = fin;
+                bra = brc; bia = bic; brc = brn; bic = bin;
             }
+        }
+        sd = nx;
+    }
+
+    // S7: exp(-2 pi i phi) = conj(q): V = (s re, -s im); coalesced float2 stores along b
+    if (valid) {
+#pragma unroll
+        for (int j = 0; j < H; ++j) {
+            float a0, a1, b0, b1;
+            unpack2(acc_re[j], a0, a1);
+            unpack2(acc_im[j], b0, b1);
+            const float sg = walk_neg(j) ? -1.f : 1.f;
+            if (p.ftile * FT + j < p.F) row[(size_t)j * p.B] = make_float2(sg * a0, -sg * b0);
+            if (p.ftile * FT + j + H < p.F) row[(size_t)(j + H) * p.B] = make_float2(sg * a1, -sg * b1);
         }
     }
 }
 
-template <bool GAUSS, typename Geo>
-cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const float *flux, int n_pad,
-                   float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
+// Fills the per-launch constant blocks: blocks[(ftile * n_chunks + chunk)] = WalkBlock<Geo>.
+// One thread per (ftile, component, flux slot); slot 0 also copies the geometry record.
+template <typename Geo>
+__global__ void pack_walk_blocks_kernel(const Geo *__restrict__ geo, const double *__restrict__ s0,
+                                        const double *__restrict__ alpha, double inv_ref, int n,
+                                        const double *__restrict__ nu, int F, int n_ftiles, int n_chunks,
+                                        unsigned char *__restrict__ blocks, unsigned int *err)
 {
-    WParams<Geo> p;
-    p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m;
-    p.geo = geo; p.flux = flux; p.chan_s = ch.s; p.vis = vis;
-    p.n_bt = (long long)uvw.T * uvw.B;
-    p.B = uvw.B; p.F = uvw.F; p.n_pad = n_pad; p.accumulate = accumulate; p.ds = ch.ds; p.err = err;
-    const int smem = WSTAGES * KB * ((int)sizeof(Geo) + WALK_FT * 4);
-    auto kern = predict_walk_kernel<GAUSS>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)((p.n_bt + PG_THREADS - 1) / PG_THREADS), (unsigned)(ch.F_pad / WALK_FT));
-    kern<<<grid, PG_THREADS, smem, st>>>(p);
-    return cudaGetLastError();
+    constexpr int KC = WalkBlock<Geo>::KC;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_ftiles * n * WALK_FT) return;
+    const int pos = (int)(i % WALK_FT);
+    const long long r = i / WALK_FT;
+    const int k = (int)(r % n), ftile = (int)(r / n);
+    const int j = (pos >> 1) + (pos & 1) * WH;               // lane 0: channel pos/2, lane 1: + WH
+    const int f = ftile * WALK_FT + j;
+    WalkBlock<Geo> *blk = reinterpret_cast<WalkBlock<Geo> *>(blocks + ((size_t)ftile * n_chunks + k / KC) * WALK_CB_BYTES);
+    float val = 0.f;
+    if (f < F) {
+        // step S2: S_k(nu_f) = s0 (nu_f / ref)^alpha in FP64, stored FP32; not finite in FP32: 0 and counted
+        const double sv = s0[k] * pow(nu[f] * inv_ref, alpha[k]);
+        if (isfinite(sv) && fabs(sv) <= 3.4028234663852886e38) val = (float)sv;
+        else atomicAdd(err, 1u);
+    }
+    reinterpret_cast<float *>(blk->rec[k % KC].flux)[pos] = val;
+    if (pos == 0) blk->rec[k % KC].geo = geo[k];
+}
+
+template <bool GAUSS, typename Geo>
+cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n, float2 *vis,
+                   int accumulate, unsigned int *err, const WalkStreams &ws)
+{
+    constexpr int KC = WalkBlock<Geo>::KC;
+    const int n_ftiles = ch.F_pad / WALK_FT, n_chunks = (n + KC - 1) / KC;
+    const long long n_bt = (long long)uvw.T * uvw.B;
+    WParams p;
+    p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m; p.vis = vis;
+    p.B = uvw.B; p.F = uvw.F; p.ds = ch.ds; p.err = err;
+
+    // Two lanes (bank half + stream each) that own disjoint outputs: whole channel tiles dealt
+    // alternately, or the two halves of the (baseline, time) range when there is one tile.
+    cudaError_t e = cudaEventRecord(ws.fork, ws.main);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ws.aux, ws.fork, 0);
+    const int n_units = n_ftiles >= 2 ? n_ftiles : 2;
+    const long long half_bt = (n_bt / 2 + WTHREADS - 1) / WTHREADS * WTHREADS;
+    for (int unit = 0; unit < n_units && e == cudaSuccess; ++unit) {
+        const int lane = unit & 1;
+        const cudaStream_t st = lane ? ws.aux : ws.main;
+        const int ftile = n_ftiles >= 2 ? unit : 0;
+        p.bt0 = n_ftiles >= 2 ? 0 : (unit == 0 ? 0 : half_bt);
+        p.bt1 = n_ftiles >= 2 ? n_bt : (unit == 0 ? (half_bt < n_bt ? half_bt : n_bt) : n_bt);
+        if (p.bt1 <= p.bt0) continue;
+        p.ftile = ftile;
+        p.sfA = ch.s_host[ftile * WALK_FT + WJ0];
+        p.sfB = ch.s_host[ftile * WALK_FT + WH + WJ0];
+        const double sa = ch.s_host[ftile * WALK_FT], sb = ch.s_host[ftile * WALK_FT + WALK_FT - 1];
+        p.smax = sa > sb ? sa : sb;
+        const unsigned grid = (unsigned)((p.bt1 - p.bt0 + WTHREADS - 1) / WTHREADS);
+        for (int c = 0; c < n_chunks && e == cudaSuccess; ++c) {
+            p.n_k = n - c * KC < KC ? n - c * KC : KC;
+            p.load_acc = (accumulate || c > 0) ? 1 : 0;
+            p.first = c == 0;
+            p.k0 = lane * KC;
+            const size_t bytes = sizeof(WalkRec<Geo>) * (size_t)p.n_k;
+            e = cudaMemcpyToSymbolAsync(CBANK, blocks + ((size_t)ftile * n_chunks + c) * WALK_CB_BYTES, bytes,
+                                        (size_t)lane * KC * sizeof(WalkRec<Geo>), cudaMemcpyDeviceToDevice, st);
+            if (e != cudaSuccess) break;
+            predict_walk_kernel<GAUSS><<<grid, WTHREADS, 0, st>>>(p);
+            e = cudaGetLastError();
+        }
+    }
+    // join even after an error so that the caller's stream stays ordered after the aux work
+    cudaError_t e2 = cudaEventRecord(ws.join, ws.aux);
+    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(ws.main, ws.join, 0);
+    return e != cudaSuccess ? e : e2;
+}
+
+template <typename Geo>
+void pack_blocks(const Geo *geo, const double *s0, const double *alpha, double ref_freq, int n, const ChanTable &ch,
+                 unsigned char *blocks, unsigned int *err, cudaStream_t st)
+{
+    constexpr int KC = WalkBlock<Geo>::KC;
+    const int n_ftiles = ch.F_pad / WALK_FT, n_chunks = (n + KC - 1) / KC;
+    const long long total = (long long)n_ftiles * n * WALK_FT;
+    pack_walk_blocks_kernel<Geo><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(geo, s0, alpha, 1.0 / ref_freq, n, ch.nu,
+                                                                                   ch.F, n_ftiles, n_chunks, blocks, err);
 }
 
 }  // namespace
 
-cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const GeoP *geo, const float *flux,
-                               int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
+size_t walk_blocks_bytes(int n, int n_ftiles, bool gauss)
 {
-    return launch<false>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
+    const int KC = gauss ? WALK_KC_GAUSS : WALK_KC_POINTS;
+    return (size_t)n_ftiles * ((n + KC - 1) / KC) * WALK_CB_BYTES;
 }
 
-cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const GeoG *geo, const float *flux,
-                                  int n_pad, float2 *vis, int accumulate, unsigned int *err, cudaStream_t st)
+void launch_pack_walk_points(const GeoP *geo, const double *s0, const double *alpha, double ref_freq, int n,
+                             const ChanTable &ch, unsigned char *blocks, unsigned int *err, cudaStream_t st)
 {
-    return launch<true>(uvw, ch, geo, flux, n_pad, vis, accumulate, err, st);
+    pack_blocks<GeoP>(geo, s0, alpha, ref_freq, n, ch, blocks, err, st);
+}
+
+void launch_pack_walk_gaussians(const GeoG *geo, const double *s0, const double *alpha, double ref_freq, int n,
+                                const ChanTable &ch, unsigned char *blocks, unsigned int *err, cudaStream_t st)
+{
+    pack_blocks<GeoG>(geo, s0, alpha, ref_freq, n, ch, blocks, err, st);
+}
+
+cudaError_t launch_walk_points(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n,
+                               float2 *vis, int accumulate, unsigned int *err, const WalkStreams &ws)
+{
+    return launch<false, GeoP>(uvw, ch, blocks, n, vis, accumulate, err, ws);
+}
+
+cudaError_t launch_walk_gaussians(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n,
+                                  float2 *vis, int accumulate, unsigned int *err, const WalkStreams &ws)
+{
+    return launch<true, GeoG>(uvw, ch, blocks, n, vis, accumulate, err, ws);
 }
 
 }  // namespace woden
