@@ -37,10 +37,16 @@ SM_COUNT = 148
 MUFU_LANES_PER_SM = 16          # measured: profiles/pipes_r1.md
 FP32_LANES_PER_SM = 128
 SM_MAX_HZ = 1965e6
-LAUNCHES_PER_STEP = {"points": 3, "gaussians": 3, "shapelets": 6}   # pack + predict kernels (+1: tensor engine)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on config 5 (profiles/ncu_r1_kernels.md)
-NCU_DRAM_BYTES = {("points", "walk"): 158166016 + 1345318912, ("gaussians", "walk"): 1536168960 + 1339894272,
-                  ("shapelets", "walk"): 1419681792 + 1340600320, ("shapelets", "general"): 1419681792 + 1340600320}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on config 5, recorded
+# from the ncu --set full captures summarised in profiles/ncu_r2_kernels.md (not measured in this run):
+# (component type, path) -> (kernel, bytes, commit the capture was taken at)
+NCU_DRAM_BYTES = {
+    ("points", "walk"): ("predict_walk_kernel<false>", 10988032 + 70947328, "5f1c2d7"),
+    ("gaussians", "walk"): ("predict_walk_kernel<true>", 10990848 + 75310080, "5f1c2d7"),
+}
+KERNEL_NAMES = {("points", "walk"): "predict_walk_kernel<false>", ("gaussians", "walk"): "predict_walk_kernel<true>",
+                ("points", "general"): "predict_pg_kernel<16, false>", ("gaussians", "general"): "predict_pg_kernel<16, true>",
+                ("shapelets", "walk"): "predict_shapelets_mma_kernel", ("shapelets", "general"): "predict_shapelets_mma_kernel"}
 
 
 def _env_int(name, default):
@@ -149,7 +155,9 @@ def run_reference(args):
         return 0
     wl = inputs.make_config(args.config)
     cores = len(os.sched_getaffinity(0))
-    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    # torchrun exports OMP_NUM_THREADS=1 to its ranks; the oracle's protocol is all cores of the
+    # affinity mask (libgomp reads the variable when the oracle library is loaded, below)
+    os.environ["OMP_NUM_THREADS"] = str(cores)
     n_sample = 1 << 14
     for i in range(args.warmup):
         time_oracle(wl, max(256, n_sample // 16), 5000 + i)
@@ -172,6 +180,57 @@ def run_reference(args):
     }
     print(json.dumps(line))
     return 0
+
+
+# ------------------------------------------------------------------------------ multi-GPU launch
+def spawn_ranks_if_needed(args):
+    """`python bench.py --gpus N` with no torchrun environment: start N ranks ourselves (one per GPU,
+    NCCL rendezvous on 127.0.0.1) by re-executing this script under torch.distributed.run.  Under
+    torchrun (WORLD_SIZE set) this is a no-op and the ranks read RANK / LOCAL_RANK / WORLD_SIZE."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return
+    import socket
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def run_dry(args):
+    """Rendezvous only (gloo, no GPU): every rank joins, the world size is all-reduced, rank 0 prints it.
+    Used by the CPU test of the --gpus N launch path."""
+    import torch
+    import torch.distributed as dist
+    rank, world = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1)
+    if world > 1:
+        dist.init_process_group("gloo")
+        t = torch.ones(1)
+        dist.all_reduce(t)
+        seen = int(t.item())
+        dist.destroy_process_group()
+    else:
+        seen = 1
+    if rank == 0:
+        print(json.dumps({"dry": True, "n_gpus": seen, "requested": args.gpus}))
+    return 0
+
+
+def time_steps(step, n_warm, n_steps, barrier):
+    """n_warm untimed + n_steps timed calls of step(record) between barriers; returns (ms_total, records)."""
+    import torch
+    for _ in range(n_warm):
+        step(None)
+    barrier()
+    recs = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_steps):
+        step(recs)
+    e1.record()
+    barrier()
+    return e0.elapsed_time(e1), recs
 
 
 # ------------------------------------------------------------------------------ our arm
@@ -237,10 +296,12 @@ def run_ours(args):
     recs = []
     e0, e1 = ev(), ev()
     barrier()
+    launches0 = binding.kernel_launches()
     e0.record()
     for _ in range(args.steps):
         step(recs)
     e1.record()
+    launches = binding.kernel_launches() - launches0       # counted by the library at every <<< >>>
     barrier()
     clocks = sampler.stop() if rank == 0 else {}
     ms_total = e0.elapsed_time(e1)
@@ -267,6 +328,16 @@ def run_ours(args):
     e2e_s = (time.perf_counter() - t0) / args.steps
     e2e_s = parallel.max_over_ranks(e2e_s, dist, f"cuda:{local}")
     e2e_value = world * evals_per_step / e2e_s
+
+    # ---- SURVEY.md 8(d) rule (ii): the general path (one sin/cos, one exp2 per eval) in the same run
+    general_ms = None
+    if args.path != "general" and not args.no_general:
+        ctx.set_path(binding.WODEN_PATH_GENERAL)
+        g_total, g_recs = time_steps(step, 3, max(3, min(5, args.steps)), barrier)
+        ctx.set_path(binding.WODEN_PATH_AUTO)
+        general_ms = {k: float(np.median([m[a].elapsed_time(m[b]) for m in g_recs]))
+                      for k, a, b in (("points", 0, 1), ("gaussians", 1, 2), ("shapelets", 2, 3))}
+        general_ms["step"] = parallel.max_over_ranks(g_total / len(g_recs), dist, f"cuda:{local}")
 
     if rank != 0:
         if dist is not None:
@@ -302,14 +373,25 @@ def run_ours(args):
            else per_type[dominant]["evals_per_s"])
     # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r1_kernels.md):
     # the visibility buffer once, plus the component blocks that miss L2
-    traffic = NCU_DRAM_BYTES.get((dominant, "walk" if walk else "general")) if args.config == 5 else None
+    key = (dominant, "walk" if walk else "general")
+    rec_traffic = NCU_DRAM_BYTES.get(key) if args.config == 5 else None
     ffma2_3reg, _ = ctx.pipe_rate("FFMA2_3REG")
+    walk_rate, _ = ctx.pipe_rate("WALK")
     roofline = {
-        "bound": "alu", "kernel": f"predict_{dominant}", "achieved": ach / 1e9, "peak": peak / 1e9,
-        "unit": "Gevals/s", "frac": ach / peak, "traffic": traffic,
+        "bound": "alu", "kernel": KERNEL_NAMES.get(key, f"predict_{dominant}"), "achieved": ach / 1e9, "peak": peak / 1e9,
+        "unit": "Gevals/s", "frac": ach / peak,
+        "traffic": rec_traffic[1] if rec_traffic else None,
+        "traffic_source": (f"ncu --set full capture of one launch of {rec_traffic[0]} at commit {rec_traffic[2]} "
+                           "(profiles/ncu_r2_kernels.md): a recorded constant, not measured in this run")
+        if rec_traffic else None,
+        "achieved_basis": "evals of the whole woden_predict_* call / its CUDA-event duration (the call is a sequence "
+                          "of launches of this kernel plus three O(K) staging kernels)",
         "operand_delivery": {"ffma2_three_fresh_pairs_fma_per_s": ffma2_3reg, "ffma_reused_operands_fma_per_s": fma_rate,
+                             "walk_pattern_fma_per_s": walk_rate,
+                             "frac_of_walk_pattern": (ach * 4.0 / walk_rate) if (walk and dominant == "points") else None,
                              "note": "register file feeds ~2 operands/clk/sub-partition: an FMA with three fresh "
-                                     "register operands runs at 2/3 of the pipe rate (DESIGN.md section 7)"},
+                                     "register operands runs at 2/3 of the pipe rate; the walking kernel's own "
+                                     "4-FFMA2 pattern in isolation sustains walk_pattern_fma_per_s (DESIGN.md section 7)"},
         "peak_basis": basis + f"; pipe rate measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
         "nominal_mufu_roofline_gevals": SM_COUNT * MUFU_LANES_PER_SM * SM_MAX_HZ / (2 if dominant == "points" else 3) / 1e9,
     }
@@ -333,10 +415,20 @@ def run_ours(args):
                         "sample": f"{n_sample} seeded random visibilities of config {wl.config}, all {comps} "
                                   f"components each ({dt:.1f} s)"}
 
-    launches = args.steps * sum(LAUNCHES_PER_STEP[k] for k in ("points", "gaussians", "shapelets")
-                                if counts[k] > 0)
-    if counts["shapelets"] > 0 and int((wl.shapelets.n1 + wl.shapelets.n2).max()) > 32:
-        launches += args.steps              # order bucket >= 40: tensor engine stages its FP16 coefficient matrices
+    general_path = None
+    if general_ms is not None:
+        general_path = {"ms_per_step": general_ms["step"], "value": world * evals_per_step / (general_ms["step"] * 1e-3),
+                        "per_type": {}, "steps": max(3, min(5, args.steps)), "warmup": 3}
+        mufu_ops = {"points": 2, "gaussians": 3}
+        for k in ("points", "gaussians", "shapelets"):
+            if counts[k] and general_ms[k]:
+                r = {"ms_per_call": general_ms[k], "evals_per_s": counts[k] / (general_ms[k] * 1e-3)}
+                if k in mufu_ops:
+                    r["frac_of_mufu_roofline"] = r["evals_per_s"] / (mufu_rate / mufu_ops[k])
+                general_path["per_type"][k] = r
+        general_path["composite_frac"] = 1e3 * t_roof / general_ms["step"]
+        general_path["note"] = ("woden_set_path(GENERAL): 2 MUFU per point eval, 3 per Gaussian eval; fractions are of the "
+                                "MUFU-pipe roofline at the pipe rate measured in this run")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -347,7 +439,7 @@ def run_ours(args):
             "l2": "no flush: each step writes 1.4 GB of visibilities, 11x the 126 MB L2; component blocks "
                   "are meant to be L2 resident",
             "parallelism": "1 GPU" if world == 1 else f"time-sharded x{world}, no collective"}),
-        "per_type": per_type, "roofline": roofline, "composite_roofline": composite,
+        "per_type": per_type, "roofline": roofline, "composite_roofline": composite, "general_path": general_path,
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "ms_per_step": 1e3 * e2e_s, "call": "woden_simulate_host (pinned host vis buffer)"},
@@ -589,6 +681,9 @@ def main():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--path", choices=["auto", "general"], default="auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-general", action="store_true", help="skip the general-path record of the line")
+    ap.add_argument("--dry", action="store_true",
+                    help="rendezvous only (gloo, no GPU work): checks that --gpus N starts N ranks")
     ap.add_argument("--pipes", action="store_true", help="print the measured pipe rates and exit")
     ap.add_argument("--only", choices=["points", "gaussians", "shapelets"], default=None,
                     help="time ONE predict call of one component type (used for the per-kernel ncu captures) and exit")
@@ -602,6 +697,9 @@ def main():
     ap.add_argument("--truncation", action="store_true",
                     help="GPU time vs kept fraction of components (PAPER.md section 5.3) and exit")
     args = ap.parse_args()
+    spawn_ranks_if_needed(args)
+    if args.dry:
+        return run_dry(args)
     if args.pipes:
         return run_pipes(args)
     if args.truncation:

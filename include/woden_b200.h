@@ -70,6 +70,10 @@ int woden_destroy(woden_ctx *ctx);
 const char *woden_strerror(int status);
 const char *woden_last_error(const woden_ctx *ctx);
 
+/* Number of CUDA kernels this library has launched since it was loaded (all contexts; copies and
+ * memsets are not counted).  Host-side counter, not thread-safe against concurrent callers. */
+unsigned long long woden_kernel_launches(void);
+
 /* Synchronises the context's last stream and reports device-side precondition violations
  * counted since the last check (l^2+m^2 >= 1, non-finite parameters, a flux s0 (nu/ref)^alpha that
  * is not finite in FP32 at any channel, negative widths, beta <= 0, shapelet orders above p_max,

@@ -37,7 +37,7 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12, "FFMA2_UR": 13, "WALK": 14}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
-           "woden_set_path", "woden_last_path", "woden_predict_points", "woden_predict_gaussians",
+           "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
            "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series"]
 
@@ -110,7 +110,10 @@ def load() -> C.CDLL:
     L.woden_calibrate_gains.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, C.c_int, _vp, _vp]
     L.woden_peel.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     for name in EXPORTS:
-        if name not in ("woden_strerror", "woden_last_error"):
+        if name == "woden_kernel_launches":
+            L.woden_kernel_launches.restype = C.c_ulonglong
+            L.woden_kernel_launches.argtypes = []
+        elif name not in ("woden_strerror", "woden_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -336,6 +339,11 @@ class Woden:
         rc = self._L.woden_pipe_rate(self._ctx, PIPES[which], int(iters), C.byref(ops), C.byref(clk))
         self._ck(rc, "woden_pipe_rate")
         return ops.value, clk.value
+
+
+def kernel_launches() -> int:
+    """Kernels launched by the library since it was loaded (woden_kernel_launches)."""
+    return int(load().woden_kernel_launches())
 
 
 class DeviceWorkload:

@@ -14,6 +14,8 @@
 
 using namespace woden;
 
+unsigned long long woden::g_kernel_launches = 0;
+
 namespace {
 
 struct DevBuf {
@@ -263,6 +265,8 @@ int woden_set_path(woden_ctx *ctx, int path)
     ctx->path = path;
     return WODEN_OK;
 }
+
+unsigned long long woden_kernel_launches(void) { return woden::g_kernel_launches; }
 
 int woden_last_path(const woden_ctx *ctx) { return ctx ? ctx->last_path : WODEN_PATH_NONE; }
 

@@ -92,7 +92,7 @@ __global__ void series_lut_kernel(const float *__restrict__ x_in, const float *_
 
 cudaError_t launch_lut_build(float2 *T, int n_x, int PM, double dx, cudaStream_t st)
 {
-    lut_build_kernel<<<(n_x + 127) / 128, 128, 0, st>>>(T, n_x, PM, dx);
+    lut_build_kernel<<<(n_x + 127) / 128, 128, 0, st>>>(T, n_x, PM, dx); note_launch();
     return cudaGetLastError();
 }
 
@@ -100,8 +100,8 @@ cudaError_t launch_series(int method, const float *x, const float *c, int PM, lo
                           double dx, float *out, cudaStream_t st)
 {
     const unsigned grid = (unsigned)((n + 255) / 256);
-    if (method == 0) series_recurrence_kernel<<<grid, 256, 0, st>>>(x, c, PM, n, out);
-    else series_lut_kernel<<<grid, 256, 0, st>>>(x, c, PM, n, T, n_x, (float)(1.0 / dx), out);
+    if (method == 0) { series_recurrence_kernel<<<grid, 256, 0, st>>>(x, c, PM, n, out); note_launch(); }
+    else { series_lut_kernel<<<grid, 256, 0, st>>>(x, c, PM, n, T, n_x, (float)(1.0 / dx), out); note_launch(); }
     return cudaGetLastError();
 }
 

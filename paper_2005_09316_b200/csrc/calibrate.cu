@@ -278,7 +278,7 @@ cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *g
     const size_t smem = calibrate_smem_bytes(N);
     cudaError_t e = cudaFuncSetAttribute(calibrate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    calibrate_kernel<<<(unsigned)cells, CAL_THREADS, smem, st>>>(p);
+    calibrate_kernel<<<(unsigned)cells, CAL_THREADS, smem, st>>>(p); note_launch();
     return cudaGetLastError();
 }
 
@@ -286,7 +286,7 @@ cudaError_t launch_peel(const float2 *data, const float2 *model, const double2 *
                         long long cells, cudaStream_t st)
 {
     const long long B = (long long)N * (N - 1) / 2;
-    peel_kernel<<<(unsigned)cells, CAL_THREADS, (size_t)N * sizeof(double2), st>>>(data, model, gains, out, N, B);
+    peel_kernel<<<(unsigned)cells, CAL_THREADS, (size_t)N * sizeof(double2), st>>>(data, model, gains, out, N, B); note_launch();
     return cudaGetLastError();
 }
 

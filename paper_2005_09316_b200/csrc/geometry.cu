@@ -81,14 +81,14 @@ cudaError_t launch_uvw(const double *X, const double *Y, const double *Z, int n_
 {
     const long long B = (long long)n_ant * (n_ant - 1) / 2;
     uvw_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(X, Y, Z, n_ant, B, T, hour_angle_dev, sin(dec0), cos(dec0),
-                                                            u, v, w);
+                                                            u, v, w); note_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_uv_basis(const double *l, const double *m, int n, double dec0, double *M, unsigned int *err,
                             cudaStream_t st)
 {
-    uv_basis_kernel<<<(n + 127) / 128, 128, 0, st>>>(l, m, n, sin(dec0), cos(dec0), M, err);
+    uv_basis_kernel<<<(n + 127) / 128, 128, 0, st>>>(l, m, n, sin(dec0), cos(dec0), M, err); note_launch();
     return cudaGetLastError();
 }
 

@@ -7,6 +7,10 @@
 
 namespace woden {
 
+// every kernel launch of the library is counted (woden_kernel_launches; bench.py's gpu_launches)
+extern unsigned long long g_kernel_launches;
+inline void note_launch() { ++g_kernel_launches; }
+
 struct UvwDev {
     const double *u_m, *v_m, *w_m;
     int B, T, F;

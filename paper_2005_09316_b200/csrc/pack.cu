@@ -204,13 +204,13 @@ inline int blocks_for(long long n, int t) { return (int)((n + t - 1) / t); }
 void launch_pack_points(const double *l, const double *m, int n, int n_pad, GeoP *geo, unsigned int *err,
                         cudaStream_t st)
 {
-    pack_points_kernel<<<blocks_for(n_pad, 256), 256, 0, st>>>(l, m, n, n_pad, geo, err);
+    pack_points_kernel<<<blocks_for(n_pad, 256), 256, 0, st>>>(l, m, n, n_pad, geo, err); note_launch();
 }
 
 void launch_pack_gaussians(const double *l, const double *m, const double *maj, const double *mnr,
                            const double *pa, int n, int n_pad, GeoG *geo, unsigned int *err, cudaStream_t st)
 {
-    pack_gaussians_kernel<<<blocks_for(n_pad, 256), 256, 0, st>>>(l, m, maj, mnr, pa, n, n_pad, geo, err);
+    pack_gaussians_kernel<<<blocks_for(n_pad, 256), 256, 0, st>>>(l, m, maj, mnr, pa, n, n_pad, geo, err); note_launch();
 }
 
 void launch_pack_flux(const double *s0, const double *alpha, double ref_freq, int n, int n_pad,
@@ -218,7 +218,7 @@ void launch_pack_flux(const double *s0, const double *alpha, double ref_freq, in
 {
     const long long total = (long long)(ch.F_pad / FT) * n_pad * FT;
     pack_flux_kernel<<<blocks_for(total, 256), 256, 0, st>>>(s0, alpha, 1.0 / ref_freq, n, n_pad, ch.nu, ch.F, FT,
-                                                             interleave ? 1 : 0, total, flux, err);
+                                                             interleave ? 1 : 0, total, flux, err); note_launch();
 }
 
 void launch_pack_shapelets(const double *l, const double *m, const double *beta1, const double *beta2,
@@ -226,19 +226,20 @@ void launch_pack_shapelets(const double *l, const double *m, const double *beta1
                            unsigned int *err, cudaStream_t st)
 {
     pack_shapelets_kernel<<<blocks_for(n, 128), 128, 0, st>>>(l, m, beta1, beta2, pa, uv_basis, n, tri_stride(PM),
-                                                              geo, err);
+                                                              geo, err); note_launch();
 }
 
 void launch_pack_coeffs(const int *coeff_offset, const int *n1, const int *n2, const double *coeff, int n,
                         int n_coeff, int p_max, int PM, float *tri, unsigned int *err, cudaStream_t st)
 {
     const long long tot = (long long)n * tri_stride(PM);
-    zero_kernel<<<blocks_for(tot, 256), 256, 0, st>>>(tri, tot);
-    if (n_coeff > 0)
+    zero_kernel<<<blocks_for(tot, 256), 256, 0, st>>>(tri, tot); note_launch();
+    if (n_coeff > 0) {
         pack_coeffs_kernel<<<blocks_for(n_coeff, 256), 256, 0, st>>>(coeff_offset, n1, n2, coeff, n, n_coeff, p_max,
-                                                                     PM, tri_stride(PM), tri, err);
+                                                                     PM, tri_stride(PM), tri, err); note_launch();
+    }
     tri_mask_kernel<<<blocks_for((long long)n * (tri_size(PM) / 4), 256), 256, 0, st>>>(tri, n, tri_size(PM),
-                                                                                         tri_stride(PM));
+                                                                                         tri_stride(PM)); note_launch();
 }
 
 }  // namespace woden

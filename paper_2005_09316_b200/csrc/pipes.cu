@@ -238,9 +238,9 @@ cudaError_t run_one(int iters, int grid, float *sink, unsigned long long *clk, f
 {
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
-    pipe_kernel<W><<<grid, PIPE_THREADS>>>(iters / 8 + 1, 1.0f, sink, clk);     // warm-up
+    pipe_kernel<W><<<grid, PIPE_THREADS>>>(iters / 8 + 1, 1.0f, sink, clk); note_launch();     // warm-up
     cudaEventRecord(e0);
-    pipe_kernel<W><<<grid, PIPE_THREADS>>>(iters, 1.0f, sink, clk);
+    pipe_kernel<W><<<grid, PIPE_THREADS>>>(iters, 1.0f, sink, clk); note_launch();
     cudaEventRecord(e1);
     cudaError_t err = cudaEventSynchronize(e1);
     if (err == cudaSuccess) err = cudaGetLastError();

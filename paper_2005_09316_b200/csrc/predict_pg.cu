@@ -181,7 +181,7 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const Geo *geo, const
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((p.n_bt + PG_THREADS - 1) / PG_THREADS), (unsigned)(ch.F_pad / FT));
-    kern<<<grid, PG_THREADS, smem, st>>>(p);
+    kern<<<grid, PG_THREADS, smem, st>>>(p); note_launch();
     return cudaGetLastError();
 }
 

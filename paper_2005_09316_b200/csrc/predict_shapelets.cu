@@ -211,8 +211,8 @@ cudaError_t launch_pm(const SParams &p, int F, bool sparse, cudaStream_t st)
 {
     constexpr int NV = nv_for(PM);
     dim3 grid((unsigned)((p.n_bt + SH_THREADS - 1) / SH_THREADS), (unsigned)((F + NV - 1) / NV));
-    if (sparse) predict_shapelets_kernel<PM, NV, true><<<grid, SH_THREADS, 0, st>>>(p);
-    else predict_shapelets_kernel<PM, NV, false><<<grid, SH_THREADS, 0, st>>>(p);
+    if (sparse) { predict_shapelets_kernel<PM, NV, true><<<grid, SH_THREADS, 0, st>>>(p); note_launch(); }
+    else { predict_shapelets_kernel<PM, NV, false><<<grid, SH_THREADS, 0, st>>>(p); note_launch(); }
     return cudaGetLastError();
 }
 

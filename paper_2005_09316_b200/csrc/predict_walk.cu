@@ -345,7 +345,7 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *
             e = cudaMemcpyToSymbolAsync(CBANK, blocks + ((size_t)ftile * n_chunks + c) * WALK_CB_BYTES, bytes,
                                         (size_t)lane * KC * sizeof(WalkRec<Geo>), cudaMemcpyDeviceToDevice, st);
             if (e != cudaSuccess) break;
-            predict_walk_kernel<GAUSS><<<grid, WTHREADS, 0, st>>>(p);
+            predict_walk_kernel<GAUSS><<<grid, WTHREADS, 0, st>>>(p); note_launch();
             e = cudaGetLastError();
         }
     }
@@ -363,7 +363,7 @@ void pack_blocks(const Geo *geo, const double *s0, const double *alpha, double r
     const int n_ftiles = ch.F_pad / WALK_FT, n_chunks = (n + KC - 1) / KC;
     const long long total = (long long)n_ftiles * n * WALK_FT;
     pack_walk_blocks_kernel<Geo><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(geo, s0, alpha, 1.0 / ref_freq, n, ch.nu,
-                                                                                   ch.F, n_ftiles, n_chunks, blocks, err);
+                                                                                   ch.F, n_ftiles, n_chunks, blocks, err); note_launch();
 }
 
 }  // namespace
