@@ -226,6 +226,47 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells,
                const float *vis_data, const float *vis_model, const double *gains,
                float *vis_out, void *cuda_stream);
 
+/* Image-space shapelet fit (SHAMFI, section 2.1, :89-102): the step
+ * that produces the coefficients woden_predict_shapelets consumes.  Eq 7 (:93): one linear equation
+ * per pixel, one unknown per basis function B_{p1,p2}, p1 + p2 <= p_max (all (p_max+1)(p_max+2)/2 of
+ * them, Eq 6, in p1-major order: (0,0), (0,1), ... (0,p_max), (1,0), ...), each basis function imaged
+ * on the pixel grid and convolved with the restoring beam (:98-100); the coefficients minimise
+ * ||b - A x||^2 (:96).  It is done for each of n_beta pairs (beta1_rad[k], beta2_rad[k]); `best`
+ * receives the index of the pair with the smallest residual (:102).  Readings (G17-G19):
+ *   basis    Bimg_{n1,n2}(l, m) = 4 ln2 / (pi beta1 beta2) h_{n1}(-a x / beta1) h_{n2}(-a y / beta2),
+ *            a = 2 sqrt(2 ln 2), x = sin(pa) (l - l0) + cos(pa) (m - m0), y = cos(pa) (l - l0) - sin(pa) (m - m0):
+ *            the function whose transform is what woden_predict_shapelets evaluates for coefficient 1,
+ *            so coeff[k] can be passed to it unchanged (s0_jy = 1, l = l0, m = m0, pa, beta1, beta2);
+ *            a pixel holds Bimg dl dm (Jy/pixel for coefficients in Jy)
+ *   beam     Eq 10's Gaussian (FWHM bmaj_rad, bmin_rad, position angle bpa_rad) sampled on a
+ *            (2 half_width + 1)^2 pixel stencil and divided by its sum; zero padding outside the image;
+ *            beam == NULL or bmaj_rad == 0: no convolution
+ *   residual sum over pixels of (P - A x)^2
+ *   weights  Eq 25 (:279): |C_{p1,p2}| sum over pixels |(G * B_{p1,p2})(x_s, y_t)|
+ * grid: pixel (s, t) is at l = l_c + (s - (n_l-1)/2) dl, m = m_c + (t - (n_m-1)/2) dm (dl, dm signed,
+ * non-zero); image: DEVICE [n_m][n_l] (index t * n_l + s).  beta1_rad, beta2_rad: HOST [n_beta], > 0.
+ * coeff: DEVICE [n_beta][P]; residual: DEVICE [n_beta]; weights: DEVICE [n_beta][P] or NULL; best:
+ * DEVICE int[1] or NULL.  n_refine: refinement passes of the normal equations with the exact FP64
+ * operator (the tensor-core Gram matrix only preconditions them); 0 selects the default (6), which
+ * reaches the FP64 least-squares solution when the scaled design matrix has a condition number
+ * below ~10^3 and otherwise still reduces the residual monotonically.  0 <= p_max <= 48
+ * (WODEN_ERR_ORDER), half_width <= 24, n_l n_m <= 2^22 (WODEN_ERR_DIM).  A Gram matrix that is not
+ * positive definite even after diagonal loading is counted for woden_check(). */
+typedef struct {
+    int n_l, n_m;
+    double dl, dm, l_c, m_c;
+} woden_image_grid;
+typedef struct {
+    double bmaj_rad, bmin_rad, bpa_rad;
+    int half_width;
+} woden_restoring_beam;
+#define WODEN_FIT_MAX_ORDER 48
+int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const double *image,
+                        double l0, double m0, double pa_rad, int p_max,
+                        int n_beta, const double *beta1_rad, const double *beta2_rad,
+                        const woden_restoring_beam *beam, int n_refine,
+                        double *coeff, double *residual, double *weights, int *best, void *cuda_stream);
+
 /* Basis-evaluation experiment: the 1-D shapelet series
  *   out[i] = sum_{p <= p_max} coeff[p] h_p(x[i]),   h_p(x) = H_p(x) exp(-x^2/2)/sqrt(2^p p!)
  * by the FP32 three-term recurrence of the predict kernels (WODEN_BASIS_RECURRENCE) or by the

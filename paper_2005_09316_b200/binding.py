@@ -33,13 +33,14 @@ WODEN_SHAPELET_REGISTER = 1
 WODEN_SHAPELET_TENSOR = 2
 WODEN_BASIS_RECURRENCE = 0
 WODEN_BASIS_LUT = 1
+WODEN_FIT_MAX_ORDER = 48
 PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA_IMM": 6, "F2F": 7,
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12, "FFMA2_UR": 13, "WALK": 14}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -65,6 +66,15 @@ class woden_shapelets_host(C.Structure):
                 ("l", _dp), ("m", _dp), ("s0_jy", _dp), ("alpha", _dp),
                 ("beta1_rad", _dp), ("beta2_rad", _dp), ("pa_rad", _dp), ("uv_basis", _dp),
                 ("coeff_offset", _ip), ("n1", _ip), ("n2", _ip), ("coeff", _dp)]
+
+
+class woden_image_grid(C.Structure):
+    _fields_ = [("n_l", C.c_int), ("n_m", C.c_int), ("dl", C.c_double), ("dm", C.c_double),
+                ("l_c", C.c_double), ("m_c", C.c_double)]
+
+
+class woden_restoring_beam(C.Structure):
+    _fields_ = [("bmaj_rad", C.c_double), ("bmin_rad", C.c_double), ("bpa_rad", C.c_double), ("half_width", C.c_int)]
 
 
 class WodenError(RuntimeError):
@@ -105,6 +115,8 @@ def load() -> C.CDLL:
                                       C.POINTER(woden_points_host), C.POINTER(woden_gaussians_host),
                                       C.POINTER(woden_shapelets_host), _vp, _vp]
     L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
+    L.woden_fit_shapelets.argtypes = [_vp, C.POINTER(woden_image_grid), _vp, C.c_double, C.c_double, C.c_double, C.c_int,
+                                      C.c_int, _dp, _dp, C.POINTER(woden_restoring_beam), C.c_int, _vp, _vp, _vp, _vp, _vp]
     L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
     L.woden_shapelet_uv_basis.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, _vp, _vp]
     L.woden_calibrate_gains.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, C.c_int, _vp, _vp]
@@ -333,6 +345,30 @@ class Woden:
                                            _stream_handle(stream))
         self._ck(rc, "woden_shapelet_series")
         return out
+
+    def fit_shapelets(self, image, dl, dm, l_c, m_c, l0, m0, pa_rad, p_max, beta1_rad, beta2_rad, beam=None,
+                      n_refine=0, want_weights=False, stream=None):
+        """woden_fit_shapelets on a float64 device image [n_m, n_l]; beam = (bmaj, bmin, bpa, half_width) or
+        None.  Returns device tensors (coeff [n_beta, P], residual [n_beta], weights or None, best int32[1])."""
+        import torch
+        if image.dtype != torch.float64 or image.dim() != 2:
+            raise ValueError("image must be a float64 [n_m, n_l] device tensor")
+        b1, b2 = _hd(np.atleast_1d(beta1_rad)), _hd(np.atleast_1d(beta2_rad))
+        if b1.shape != b2.shape:
+            raise ValueError("beta1_rad and beta2_rad must have one length")
+        n_beta, P = int(b1.shape[0]), (p_max + 1) * (p_max + 2) // 2
+        grid = woden_image_grid(int(image.shape[1]), int(image.shape[0]), float(dl), float(dm), float(l_c), float(m_c))
+        cb = woden_restoring_beam(*[float(x) for x in beam[:3]], int(beam[3])) if beam is not None else None
+        coeff = torch.empty((n_beta, P), dtype=torch.float64, device=image.device)
+        resid = torch.empty(n_beta, dtype=torch.float64, device=image.device)
+        weights = torch.empty_like(coeff) if want_weights else None
+        best = torch.empty(1, dtype=torch.int32, device=image.device)
+        rc = self._L.woden_fit_shapelets(self._ctx, C.byref(grid), _ptr(image), float(l0), float(m0), float(pa_rad),
+                                         int(p_max), n_beta, _hdp(b1), _hdp(b2), C.byref(cb) if cb is not None else None,
+                                         int(n_refine), _ptr(coeff), _ptr(resid), _ptr(weights), _ptr(best),
+                                         _stream_handle(stream))
+        self._ck(rc, "woden_fit_shapelets")
+        return coeff, resid, weights, best
 
     def pipe_rate(self, which: str, iters: int = 20000):
         ops, clk = C.c_double(0.0), C.c_double(0.0)

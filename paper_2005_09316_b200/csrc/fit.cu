@@ -1,0 +1,576 @@
+// fit.cu -- image-space shapelet fit (SHAMFI, section 2.1, :89-102).
+//
+// Eq 7 (:93): one linear equation per pixel, one unknown per basis function B_{p1,p2}, p1 + p2 <= p_max,
+// each basis function imaged on the pixel grid and convolved with the restoring beam (:98-100); the
+// coefficients minimise ||b - A x||^2 (:96); a list of (beta1, beta2) pairs is searched by the residual
+// of each fit (:102).  Eq 25 (:279): truncation weight of a basis function = sum over pixels of
+// |C (G * B)|.  Image basis, beam stencil and residual follow DESIGN.md readings G17-G19.
+//
+// How it is computed here (the oracle calls numpy.linalg.lstsq on the explicit matrix; this is a
+// different route to the same least-squares solution):
+//   1. basis:   h_p(-a x/beta1), h_p(-a y/beta2) for every pixel by the normalised three-term recurrence
+//               in FP64; At[q][i] = norm h_{n1}(x_i) h_{n2}(y_i) (basis-major, pixel contiguous).
+//   2. beam:    direct 2-D convolution of every basis image with the unit-sum stencil, FP64.
+//   3. scaling: every row of At is scaled by a power of two to max |.| in [1/2, 1) (the unknowns become
+//               z = x / scale); row sums of |At| give the Eq 25 weights.
+//   4. Gram:    G = At At^T, the one dense contraction of the path (pixels are the K dimension,
+//               tens of thousands x ~10^3 basis functions), on the tensor cores: tcgen05.mma kind::f16,
+//               operands split FP16 hi + lo (three products, ~22 bits), FP32 accumulation in TMEM over a
+//               K range per CTA, K-split partials summed in FP64 in a fixed order.  Operand tiles are
+//               staged through a 3-stage ring of bulk async copies (TMA engine) on mbarriers; one thread
+//               issues the MMAs and releases stages with tcgen05.commit.
+//   5. solve:   Cholesky of G + ridge (FP64, one CTA), then iterative refinement on the normal
+//               equations with the EXACT FP64 operator: z += (L L^T)^-1 At (b - At^T z).  The Gram matrix
+//               only preconditions; the fixed point is the least-squares solution of the FP64 system.
+//   6. outputs: x = scale z, residual = ||b - At^T z||^2, weights, arg-min over the beta list.
+#include <cuda_fp16.h>
+
+#include <cmath>
+
+#include "kernels.h"
+#include "ptx.cuh"
+
+namespace woden {
+namespace {
+
+constexpr double LN2 = 0.693147180559945309417232121458176568;
+constexpr double PI = 3.14159265358979323846264338327950288;
+
+// ---------------------------------------------------------------------------------- 1. basis
+struct BasisParams {
+    int n_l, n_m, p_max;
+    double dl, dm, l_c, m_c, l0, m0, sp, cp;      // sin / cos of the position angle
+    double ax, ay;                                 // -a / beta1, -a / beta2 (reading G17: reflected)
+};
+
+// hx[p][i], hy[p][i]: h_p at the pixel's scaled, rotated coordinates (h_p = H_p exp(-t^2/2)/sqrt(2^p p!))
+__global__ void fit_hermite_kernel(const BasisParams b, double *__restrict__ hx, double *__restrict__ hy)
+{
+    const int n_pix = b.n_l * b.n_m;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pix) return;
+    const int s = i % b.n_l, t = i / b.n_l;
+    const double l = b.l_c + (s - 0.5 * (b.n_l - 1)) * b.dl - b.l0;
+    const double m = b.m_c + (t - 0.5 * (b.n_m - 1)) * b.dm - b.m0;
+    const double tx = b.ax * (b.sp * l + b.cp * m);       // along the major axis (reading G7)
+    const double ty = b.ay * (b.cp * l - b.sp * m);
+#pragma unroll
+    for (int which = 0; which < 2; ++which) {
+        const double x = which ? ty : tx;
+        double *out = which ? hy : hx;
+        double hm = 0.0, hc = exp(-0.5 * x * x);
+        out[i] = hc;
+        for (int p = 0; p < b.p_max; ++p) {
+            const double hn = sqrt(2.0 / (p + 1.0)) * x * hc - sqrt(p / (p + 1.0)) * hm;
+            hm = hc; hc = hn;
+            out[(size_t)(p + 1) * n_pix + i] = hn;
+        }
+    }
+}
+
+// At[q][i] = norm hx[n1_q][i] hy[n2_q][i], q in full-triangle (n1-major) order
+__global__ void fit_product_kernel(const double *__restrict__ hx, const double *__restrict__ hy, int n_pix, int p_max,
+                                   int P, double norm, double *__restrict__ At)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int q = blockIdx.y;
+    if (i >= n_pix || q >= P) return;
+    // invert q -> (n1, n2): rows n1 = 0.. hold p_max + 1 - n1 entries
+    int n1 = 0, off = 0;
+    while (off + (p_max + 1 - n1) <= q) { off += p_max + 1 - n1; ++n1; }
+    const int n2 = q - off;
+    At[(size_t)q * n_pix + i] = norm * hx[(size_t)n1 * n_pix + i] * hy[(size_t)n2 * n_pix + i];
+}
+
+// ---------------------------------------------------------------------------------- 2. beam
+// stencil[(dt + hw) * (2hw+1) + (ds + hw)] = Eq 10 at the pixel offset, divided by the sum (one CTA)
+__global__ void fit_stencil_kernel(double dl, double dm, double bmaj, double bmin, double sb, double cb, int hw,
+                                   double *__restrict__ stencil)
+{
+    __shared__ double red[256];
+    const int w = 2 * hw + 1, n = w * w;
+    double part = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const double ol = (k % w - hw) * dl, om = (k / w - hw) * dm;
+        const double xb = sb * ol + cb * om, yb = cb * ol - sb * om;
+        const double ex = bmaj > 0.0 ? xb * xb / (bmaj * bmaj) : (xb == 0.0 ? 0.0 : INFINITY);
+        const double ey = bmin > 0.0 ? yb * yb / (bmin * bmin) : (yb == 0.0 ? 0.0 : INFINITY);
+        const double v = exp(-4.0 * LN2 * (ex + ey));
+        stencil[k] = v;
+        part += v;
+    }
+    red[threadIdx.x] = part;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    const double inv = 1.0 / red[0];
+    for (int k = threadIdx.x; k < n; k += blockDim.x) stencil[k] *= inv;
+}
+
+// out[q][t][s] = sum_{dt, ds} stencil[dt][ds] in[q][t - dt][s - ds], zero outside the image.
+// One CTA = one basis image row-block of 16 x 16 output pixels; the stencil is centro-symmetric, so
+// correlation and convolution coincide.
+__global__ void fit_convolve_kernel(const double *__restrict__ in, const double *__restrict__ stencil, int n_l, int n_m,
+                                    int hw, double *__restrict__ out)
+{
+    extern __shared__ double sm[];
+    const int w = 2 * hw + 1, tile = 16 + 2 * hw;
+    double *st = sm, *patch = sm + w * w;
+    const int q = blockIdx.z, s0 = blockIdx.x * 16, t0 = blockIdx.y * 16;
+    const double *img = in + (size_t)q * n_l * n_m;
+    const int tid = threadIdx.y * 16 + threadIdx.x;
+    for (int k = tid; k < w * w; k += 256) st[k] = stencil[k];
+    for (int k = tid; k < tile * tile; k += 256) {
+        const int s = s0 - hw + k % tile, t = t0 - hw + k / tile;
+        patch[k] = (s >= 0 && s < n_l && t >= 0 && t < n_m) ? img[(size_t)t * n_l + s] : 0.0;
+    }
+    __syncthreads();
+    const int s = s0 + threadIdx.x, t = t0 + threadIdx.y;
+    if (s >= n_l || t >= n_m) return;
+    double acc = 0.0;
+    for (int dt = 0; dt < w; ++dt)
+        for (int ds = 0; ds < w; ++ds)
+            acc = fma(st[dt * w + ds], patch[(threadIdx.y + 2 * hw - dt) * tile + threadIdx.x + 2 * hw - ds], acc);
+    out[(size_t)q * n_l * n_m + (size_t)t * n_l + s] = acc;
+}
+
+// ---------------------------------------------------------------------------------- 3. scaling
+// per row q: scale[q] = 2^-e with max|At[q]| = f 2^e, f in [1/2, 1) (1 for an all-zero row);
+// abssum[q] = sum_i |At[q][i]| (Eq 25); the row is scaled in place.
+__global__ void fit_scale_rows_kernel(double *__restrict__ At, int n_pix, double *__restrict__ scale,
+                                      double *__restrict__ abssum)
+{
+    __shared__ double red_m[256], red_s[256];
+    double *row = At + (size_t)blockIdx.x * n_pix;
+    double mx = 0.0, sum = 0.0;
+    for (int i = threadIdx.x; i < n_pix; i += blockDim.x) { const double a = fabs(row[i]); mx = fmax(mx, a); sum += a; }
+    red_m[threadIdx.x] = mx; red_s[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            red_m[threadIdx.x] = fmax(red_m[threadIdx.x], red_m[threadIdx.x + o]);
+            red_s[threadIdx.x] += red_s[threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    int e = 0;
+    if (red_m[0] > 0.0 && isfinite(red_m[0])) frexp(red_m[0], &e);
+    const double sc = ldexp(1.0, -e);
+    if (threadIdx.x == 0) { scale[blockIdx.x] = sc; abssum[blockIdx.x] = red_s[0]; }
+    for (int i = threadIdx.x; i < n_pix; i += blockDim.x) row[i] *= sc;
+}
+
+// ---------------------------------------------------------------------------------- 4. Gram on tcgen05
+constexpr int GT = 128;                  // tile rows (UMMA M = N = 128)
+constexpr int GK = 64;                   // pixels per pipeline stage (4 UMMA K steps of 16)
+constexpr int GSTAGES = 3;
+constexpr int G_BLOCK_BYTES = GT * GK * 2;            // one operand tile of one stage: 16 KB
+constexpr int G_STAGE_BYTES = 4 * G_BLOCK_BYTES;      // A hi, A lo, B hi, B lo
+
+// FP16 hi + lo of the scaled rows in the tcgen05 no-swizzle K-major core-matrix layout, blocked so that
+// one (k tile, row tile) operand block is 16 KB contiguous: halves[part][kt][rt][k8][row][8].
+__global__ void fit_split_kernel(const double *__restrict__ At, int P, int n_pix, int n_rt, int n_kt,
+                                 __half *__restrict__ ops)
+{
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // (row, 8-pixel group)
+    const int n_k8 = n_kt * (GK / 8);
+    if (g >= (long long)n_rt * GT * n_k8) return;
+    const int row = (int)(g / n_k8), k8g = (int)(g % n_k8);
+    __align__(16) __half hi[8], lo[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const int i = k8g * 8 + j;
+        const double v = (row < P && i < n_pix) ? At[(size_t)row * n_pix + i] : 0.0;
+        const float f = (float)v;
+        hi[j] = __float2half_rn(f);
+        lo[j] = __float2half_rn((float)(v - (double)__half2float(hi[j])));
+    }
+    const int kt = k8g / (GK / 8), k8 = k8g % (GK / 8), rt = row / GT, r = row % GT;
+    const size_t blk = ((size_t)kt * n_rt + rt) * (GK / 8) + k8;
+    const size_t part = (size_t)n_kt * n_rt * GT * GK;
+    *reinterpret_cast<uint4 *>(ops + (blk * GT + r) * 8) = *reinterpret_cast<const uint4 *>(hi);
+    *reinterpret_cast<uint4 *>(ops + part + (blk * GT + r) * 8) = *reinterpret_cast<const uint4 *>(lo);
+}
+
+struct GramParams {
+    const __half *ops;       // [2][n_kt][n_rt][8][128][8]
+    float *partial;          // [n_split][n_pairs][128][128]
+    int n_rt, n_kt, n_pairs, kt_per_split;
+};
+
+// One CTA = one tile pair (ti <= tj) x one K split: D[128 x 128] = sum over its k tiles of A_ti B_tj^T.
+__global__ void __launch_bounds__(128) fit_gram_kernel(const GramParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t full_bar[GSTAGES], empty_bar[GSTAGES], done_bar;
+    __shared__ uint32_t tmem_holder;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // tile pair index -> (ti, tj), ti <= tj
+    int ti = 0, rem = blockIdx.x;
+    while (rem >= p.n_rt - ti) { rem -= p.n_rt - ti; ++ti; }
+    const int tj = ti + rem;
+    const int kt0 = blockIdx.y * p.kt_per_split;
+    const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
+    const int n_it = kt1 - kt0;
+
+    if (warp == 0) tmem_alloc(&tmem_holder, 128);
+    if (tid == 0) {
+        for (int s = 0; s < GSTAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+        mbar_init(&done_bar, 1);
+        fence_mbar_init();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_holder;
+    const size_t part = (size_t)p.n_kt * p.n_rt * GT * GK;        // halves per hi / lo part
+
+    if (warp == 0 && lane == 0) {
+        // producer: four 16 KB bulk copies per stage
+        for (int it = 0; it < n_it; ++it) {
+            const int s = it % GSTAGES;
+            if (it >= GSTAGES) mbar_wait(&empty_bar[s], ((it / GSTAGES) - 1) & 1);
+            unsigned char *dst = smem + (size_t)s * G_STAGE_BYTES;
+            const size_t a_off = ((size_t)(kt0 + it) * p.n_rt + ti) * GT * GK, b_off = ((size_t)(kt0 + it) * p.n_rt + tj) * GT * GK;
+            mbar_arrive_expect_tx(&full_bar[s], G_STAGE_BYTES);
+            bulk_g2s(dst, p.ops + a_off, G_BLOCK_BYTES, &full_bar[s]);
+            bulk_g2s(dst + G_BLOCK_BYTES, p.ops + part + a_off, G_BLOCK_BYTES, &full_bar[s]);
+            bulk_g2s(dst + 2 * G_BLOCK_BYTES, p.ops + b_off, G_BLOCK_BYTES, &full_bar[s]);
+            bulk_g2s(dst + 3 * G_BLOCK_BYTES, p.ops + part + b_off, G_BLOCK_BYTES, &full_bar[s]);
+        }
+    } else if (warp == 1 && lane == 0) {
+        // MMA issuer: 4 K steps x (hi hi + hi lo + lo hi) per stage, then release the stage
+        const uint32_t idesc = umma_idesc_f16(GT, GT);
+        const uint32_t lbo = GT * 16, sbo = 128;                   // K-chunk stride, 8-row group stride
+        for (int it = 0; it < n_it; ++it) {
+            const int s = it % GSTAGES;
+            mbar_wait(&full_bar[s], (it / GSTAGES) & 1);
+            tc_fence_after();
+            const uint32_t base = smem_u32(smem + (size_t)s * G_STAGE_BYTES);
+#pragma unroll
+            for (int ks = 0; ks < GK / 16; ++ks) {
+                const uint32_t ko = (uint32_t)ks * 2u * lbo;       // two 16-byte K chunks per step
+                const uint64_t aH = umma_desc_kmajor(base + ko, lbo, sbo);
+                const uint64_t aL = umma_desc_kmajor(base + G_BLOCK_BYTES + ko, lbo, sbo);
+                const uint64_t bH = umma_desc_kmajor(base + 2 * G_BLOCK_BYTES + ko, lbo, sbo);
+                const uint64_t bL = umma_desc_kmajor(base + 3 * G_BLOCK_BYTES + ko, lbo, sbo);
+                umma_f16(tmem, aH, bH, idesc, (it > 0 || ks > 0) ? 1u : 0u);
+                umma_f16(tmem, aH, bL, idesc, 1u);
+                umma_f16(tmem, aL, bH, idesc, 1u);
+            }
+            umma_commit(&empty_bar[s]);                            // arrives when these MMAs have read smem
+        }
+        umma_commit(&done_bar);
+    }
+    __syncwarp();
+    // epilogue: every thread reads its TMEM lane (= tile row) and writes the FP32 partial
+    if (n_it > 0) {
+        mbar_wait(&done_bar, 0);
+        tc_fence_after();
+    }
+    float *dst = p.partial + (((size_t)blockIdx.y * p.n_pairs + blockIdx.x) * GT + tid) * GT;
+    const uint32_t lane_base = tmem + ((uint32_t)(warp * 32) << 16);
+#pragma unroll 1
+    for (int c = 0; c < GT; c += 16) {
+        uint32_t v[16];
+        if (n_it > 0) { tmem_ld16_issue(lane_base + (uint32_t)c, v); tmem_ld_wait(); }
+        else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[j] = 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < 16; j += 4)
+            *reinterpret_cast<uint4 *>(dst + c + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, 128);
+}
+
+// G[r][c] = sum over splits (fixed order, FP64) of the tile partials, mirrored to the full matrix;
+// + ridge on the diagonal; rows >= P (padding) become identity rows.
+__global__ void fit_gram_reduce_kernel(const float *__restrict__ partial, int n_split, int n_pairs, int n_rt, int P,
+                                       double ridge, double *__restrict__ G)
+{
+    const int n = n_rt * GT;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y;
+    if (c >= n || c < r) return;                                 // upper triangle incl. diagonal: r <= c
+    const int ti = r / GT, tj = c / GT;
+    int pair = 0;
+    for (int t = 0; t < ti; ++t) pair += n_rt - t;
+    pair += tj - ti;
+    double s = 0.0;
+    for (int k = 0; k < n_split; ++k)
+        s += (double)partial[(((size_t)k * n_pairs + pair) * GT + (r % GT)) * GT + (c % GT)];
+    if (r >= P || c >= P) s = (r == c) ? 1.0 : 0.0;
+    else if (r == c) s += ridge * s;
+    G[(size_t)r * n + c] = s;
+    G[(size_t)c * n + r] = s;
+}
+
+// ---------------------------------------------------------------------------------- 5. solve
+// In-place Cholesky G = L L^T by one CTA: on return the lower triangle holds L and the upper triangle
+// L^T (so that both triangular solves read rows).  Left-looking, one warp per row of the column.
+__global__ void __launch_bounds__(1024) fit_cholesky_kernel(double *__restrict__ G, int n, unsigned int *__restrict__ err)
+{
+    __shared__ double col_s[FIT_MAX_N];                          // s_i of the current column, i >= j
+    __shared__ double piv;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    for (int j = 0; j < n; ++j) {
+        const double *Lj = G + (size_t)j * n;
+        // s_i = G[i][j] - sum_{k<j} L[i][k] L[j][k] for i >= j
+        for (int i = j + warp; i < n; i += n_warps) {
+            const double *Li = G + (size_t)i * n;
+            double s = 0.0;
+            for (int k = lane; k < j; k += 32) s = fma(Li[k], Lj[k], s);
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) col_s[i - j] = Li[j] - s;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double d = col_s[0];
+            if (!(d > 0.0)) { atomicAdd(err, 1u); d = 1.0; }      // not positive definite: counted (woden_check), kept finite
+            piv = sqrt(d);
+        }
+        __syncthreads();
+        const double inv = 1.0 / piv;
+        for (int i = j + threadIdx.x; i < n; i += blockDim.x) {
+            const double v = (i == j) ? piv : col_s[i - j] * inv;
+            G[(size_t)i * n + j] = v;
+            G[(size_t)j * n + i] = v;
+        }
+        __syncthreads();
+    }
+}
+
+// z += (L L^T)^-1 g by one CTA (n <= FIT_MAX_N): forward then backward substitution, 32 rows per step:
+// the rows' dots over the already solved part run one warp per row, the 32 x 32 diagonal block is
+// finished by warp 0.
+__global__ void __launch_bounds__(1024) fit_solve_kernel(const double *__restrict__ G, int n, const double *__restrict__ g,
+                                                         double *__restrict__ z)
+{
+    __shared__ double y[FIT_MAX_N], part[32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = g[i];
+    __syncthreads();
+    // forward: L y = g (lower triangle, rows)
+    for (int r0 = 0; r0 < n; r0 += 32) {
+        const int i = r0 + warp;
+        if (i < n) {
+            const double *Li = G + (size_t)i * n;
+            double s = 0.0;
+            for (int k = lane; k < r0; k += 32) s = fma(Li[k], y[k], s);
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) part[warp] = y[i] - s;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const int rows = min(32, n - r0);
+            double v = lane < rows ? part[lane] : 0.0;
+            for (int c = 0; c < rows; ++c) {
+                const double d = G[(size_t)(r0 + c) * n + r0 + c];
+                const double yc = __shfl_sync(0xffffffffu, v, c) / d;
+                if (lane == c) v = yc;
+                else if (lane > c && lane < rows) v -= G[(size_t)(r0 + lane) * n + r0 + c] * yc;
+            }
+            if (lane < rows) y[r0 + lane] = v;
+        }
+        __syncthreads();
+    }
+    // backward: L^T x = y (upper triangle holds L^T, rows), blocks from the bottom
+    const int n_blocks = (n + 31) / 32;
+    for (int b = n_blocks - 1; b >= 0; --b) {
+        const int r0 = b * 32, r1 = min(n, r0 + 32);
+        const int i = r0 + warp;
+        if (i < r1) {
+            const double *Ui = G + (size_t)i * n;
+            double s = 0.0;
+            for (int k = r1 + lane; k < n; k += 32) s = fma(Ui[k], y[k], s);
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) part[warp] = y[i] - s;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const int rows = r1 - r0;
+            double v = lane < rows ? part[lane] : 0.0;
+            for (int c = rows - 1; c >= 0; --c) {
+                const double d = G[(size_t)(r0 + c) * n + r0 + c];
+                const double xc = __shfl_sync(0xffffffffu, v, c) / d;
+                if (lane == c) v = xc;
+                else if (lane < c) v -= G[(size_t)(r0 + lane) * n + r0 + c] * xc;
+            }
+            if (lane < rows) y[r0 + lane] = v;
+        }
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) z[i] += y[i];
+}
+
+// r[i] = b[i] - sum_q At[q][i] z[q]   (FP64; coalesced over pixels)
+__global__ void fit_residual_kernel(const double *__restrict__ At, const double *__restrict__ z, const double *__restrict__ b,
+                                    int P, int n_pix, double *__restrict__ r)
+{
+    extern __shared__ double zs[];
+    for (int q = threadIdx.x; q < P; q += blockDim.x) zs[q] = z[q];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pix) return;
+    double s0 = 0.0, s1 = 0.0;
+    int q = 0;
+    for (; q + 1 < P; q += 2) {
+        s0 = fma(At[(size_t)q * n_pix + i], zs[q], s0);
+        s1 = fma(At[(size_t)(q + 1) * n_pix + i], zs[q + 1], s1);
+    }
+    if (q < P) s0 = fma(At[(size_t)q * n_pix + i], zs[q], s0);
+    r[i] = b[i] - (s0 + s1);
+}
+
+// g[q] = sum_i At[q][i] r[i] (one CTA per row, fixed-order tree); rows >= P of g are zero
+__global__ void fit_atr_kernel(const double *__restrict__ At, const double *__restrict__ r, int P, int n_pix,
+                               double *__restrict__ g)
+{
+    __shared__ double red[256];
+    const int q = blockIdx.x;
+    double s = 0.0;
+    if (q < P) {
+        const double *row = At + (size_t)q * n_pix;
+        for (int i = threadIdx.x; i < n_pix; i += blockDim.x) s = fma(row[i], r[i], s);
+    }
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) g[q] = red[0];
+}
+
+// ---------------------------------------------------------------------------------- 6. outputs
+// coeff[q] = scale[q] z[q]; weights[q] = |z[q]| abssum_scaled[q]... (abssum was taken before scaling:
+// |x_q| sum_i |A[q][i]| = |z_q scale_q| abssum[q]); residual = sum r^2 (one CTA, fixed order)
+__global__ void fit_finish_kernel(const double *__restrict__ z, const double *__restrict__ scale,
+                                  const double *__restrict__ abssum, const double *__restrict__ r, int P, int n_pix,
+                                  double *__restrict__ coeff, double *__restrict__ weights, double *__restrict__ residual)
+{
+    __shared__ double red[1024];
+    for (int q = threadIdx.x; q < P; q += blockDim.x) {
+        const double x = scale[q] * z[q];
+        coeff[q] = x;
+        if (weights) weights[q] = fabs(x) * abssum[q];
+    }
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n_pix; i += blockDim.x) s = fma(r[i], r[i], s);
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *residual = red[0];
+}
+
+__global__ void fit_argmin_kernel(const double *__restrict__ residual, int n, int *__restrict__ best)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    int b = 0;
+    for (int k = 1; k < n; ++k)
+        if (residual[k] < residual[b]) b = k;                    // first minimum, like numpy.argmin
+    *best = b;
+}
+
+__global__ void fit_zero_kernel(double *__restrict__ p, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = 0.0;
+}
+
+}  // namespace
+
+FitSizes fit_sizes(int n_pix, int p_max)
+{
+    FitSizes s;
+    s.P = (p_max + 1) * (p_max + 2) / 2;
+    s.n_rt = (s.P + GT - 1) / GT;
+    s.n_pad = s.n_rt * GT;
+    s.n_kt = (n_pix + GK - 1) / GK;
+    s.n_pairs = s.n_rt * (s.n_rt + 1) / 2;
+    // K splits: enough CTAs for two waves of the 148 SMs, at least 4 stages each
+    int split = (2 * 148 + s.n_pairs - 1) / s.n_pairs;
+    const int max_split = (s.n_kt + 3) / 4;
+    if (split > max_split) split = max_split;
+    if (split < 1) split = 1;
+    s.kt_per_split = (s.n_kt + split - 1) / split;
+    s.n_split = (s.n_kt + s.kt_per_split - 1) / s.kt_per_split;
+    s.hermite_doubles = (size_t)2 * (p_max + 1) * n_pix;
+    s.at_doubles = (size_t)s.P * n_pix;
+    s.ops_halves = (size_t)2 * s.n_kt * s.n_rt * GT * GK;
+    s.partial_floats = (size_t)s.n_split * s.n_pairs * GT * GT;
+    s.gram_doubles = (size_t)s.n_pad * s.n_pad;
+    return s;
+}
+
+cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st)
+{
+    const int n_pix = f.n_l * f.n_m;
+    const FitSizes sz = fit_sizes(n_pix, f.p_max);
+    const int P = sz.P;
+    const double a = 2.0 * sqrt(2.0 * LN2);
+    BasisParams b;
+    b.n_l = f.n_l; b.n_m = f.n_m; b.p_max = f.p_max;
+    b.dl = f.dl; b.dm = f.dm; b.l_c = f.l_c; b.m_c = f.m_c; b.l0 = f.l0; b.m0 = f.m0;
+    b.sp = sin(f.pa); b.cp = cos(f.pa);
+    b.ax = -a / f.beta1; b.ay = -a / f.beta2;
+    fit_hermite_kernel<<<(n_pix + 127) / 128, 128, 0, st>>>(b, w.hx, w.hx + (size_t)(f.p_max + 1) * n_pix); note_launch();
+    const double norm = 4.0 * LN2 / (PI * f.beta1 * f.beta2) * fabs(f.dl * f.dm);
+    const bool beam = f.bmaj > 0.0;
+    double *unconv = beam ? w.a0 : w.at;
+    fit_product_kernel<<<dim3((n_pix + 255) / 256, P), 256, 0, st>>>(w.hx, w.hx + (size_t)(f.p_max + 1) * n_pix, n_pix,
+                                                                      f.p_max, P, norm, unconv); note_launch();
+    if (beam) {
+        const int hw = f.half_width, wd = 2 * hw + 1, tile = 16 + 2 * hw;
+        const size_t smem = ((size_t)wd * wd + (size_t)tile * tile) * sizeof(double);
+        cudaError_t e = cudaFuncSetAttribute(fit_convolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        fit_stencil_kernel<<<1, 256, 0, st>>>(f.dl, f.dm, f.bmaj, f.bmin, sin(f.bpa), cos(f.bpa), hw, w.stencil); note_launch();
+        fit_convolve_kernel<<<dim3((f.n_l + 15) / 16, (f.n_m + 15) / 16, P), dim3(16, 16), smem, st>>>(w.a0, w.stencil, f.n_l,
+                                                                                                      f.n_m, hw, w.at); note_launch();
+    }
+    fit_scale_rows_kernel<<<P, 256, 0, st>>>(w.at, n_pix, w.scale, w.abssum); note_launch();
+    {
+        const long long groups = (long long)sz.n_pad * sz.n_kt * (GK / 8);
+        fit_split_kernel<<<(unsigned)((groups + 255) / 256), 256, 0, st>>>(w.at, P, n_pix, sz.n_rt, sz.n_kt, w.ops); note_launch();
+    }
+    GramParams gp;
+    gp.ops = w.ops; gp.partial = w.partial; gp.n_rt = sz.n_rt; gp.n_kt = sz.n_kt; gp.n_pairs = sz.n_pairs;
+    gp.kt_per_split = sz.kt_per_split;
+    const int gsmem = GSTAGES * G_STAGE_BYTES;
+    cudaError_t e = cudaFuncSetAttribute(fit_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, gsmem);
+    if (e != cudaSuccess) return e;
+    fit_gram_kernel<<<dim3(sz.n_pairs, sz.n_split), 128, gsmem, st>>>(gp); note_launch();
+    // relative diagonal loading: the split-FP16 Gram matrix carries ~2^-21 sqrt(G_rr G_cc) of error per
+    // entry; loading the diagonal by 2^-14 keeps the preconditioner positive definite for ~10^3 unknowns
+    const double ridge = ldexp(1.0, -14);
+    fit_gram_reduce_kernel<<<dim3((sz.n_pad + 127) / 128, sz.n_pad), 128, 0, st>>>(w.partial, sz.n_split, sz.n_pairs, sz.n_rt,
+                                                                                  P, ridge, w.gram); note_launch();
+    fit_cholesky_kernel<<<1, 1024, 0, st>>>(w.gram, sz.n_pad, w.err); note_launch();
+    fit_zero_kernel<<<(sz.n_pad + 255) / 256, 256, 0, st>>>(w.z, sz.n_pad); note_launch();
+    for (int it = 0; it <= f.n_refine; ++it) {
+        fit_residual_kernel<<<(n_pix + 127) / 128, 128, P * sizeof(double), st>>>(w.at, w.z, f.image, P, n_pix, w.r); note_launch();
+        if (it == f.n_refine) break;
+        fit_atr_kernel<<<sz.n_pad, 256, 0, st>>>(w.at, w.r, P, n_pix, w.g); note_launch();
+        fit_solve_kernel<<<1, 1024, 0, st>>>(w.gram, sz.n_pad, w.g, w.z); note_launch();
+    }
+    fit_finish_kernel<<<1, 1024, 0, st>>>(w.z, w.scale, w.abssum, w.r, P, n_pix, f.coeff, f.weights, f.residual); note_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fit_argmin(const double *residual, int n, int *best, cudaStream_t st)
+{
+    fit_argmin_kernel<<<1, 32, 0, st>>>(residual, n, best); note_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace woden

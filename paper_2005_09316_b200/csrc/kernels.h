@@ -95,6 +95,28 @@ cudaError_t launch_lut_build(float2 *T, int n_x, int PM, double dx, cudaStream_t
 cudaError_t launch_series(int method, const float *x, const float *c, int PM, long long n, const float2 *T, int n_x,
                           double dx, float *out, cudaStream_t st);
 
+// ---- image-space shapelet fit (fit.cu) ------------------
+constexpr int FIT_MAX_N = 1280;          // padded unknowns the single-CTA factorisation handles (p_max <= 48)
+struct FitSizes {
+    int P, n_rt, n_pad, n_kt, n_pairs, n_split, kt_per_split;
+    size_t hermite_doubles, at_doubles, ops_halves, partial_floats, gram_doubles;
+};
+FitSizes fit_sizes(int n_pix, int p_max);
+struct FitProblem {                      // one (beta1, beta2) pair
+    int n_l, n_m, p_max, half_width, n_refine;
+    double dl, dm, l_c, m_c, l0, m0, pa, beta1, beta2, bmaj, bmin, bpa;
+    const double *image;                 // [n_m][n_l]
+    double *coeff, *weights, *residual;  // [P], [P] or NULL, [1]
+};
+struct FitScratch {
+    double *hx, *a0, *at, *stencil, *scale, *abssum, *gram, *z, *g, *r;
+    __half *ops;
+    float *partial;
+    unsigned int *err;
+};
+cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st);
+cudaError_t launch_fit_argmin(const double *residual, int n, int *best, cudaStream_t st);
+
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
 
