@@ -672,6 +672,74 @@ def run_peel(args):
     return 0
 
 
+def run_fit(args):
+    """NEXT-4: the image-space shapelet fit on a synthetic restored image: a planted
+    p_max = 40 model (861 basis functions, the order of config 5's shapelets) rendered through
+    woden_fit_shapelets' own inverse is not available, so the image is a sum of seeded Gaussian blobs
+    (device-made, no oracle); 256 x 256 pixels, restoring beam of 3 pixels FWHM, 3 x 3 grid of (beta1, beta2).
+    Reports the whole call and the roofline of its dense contraction, the Gram-matrix kernel."""
+    import torch
+    from paper_2005_09316_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --fit: no CUDA device")
+    ctx = binding.Woden(0)
+    n, pix, p_max = args.fit_pixels, 0.3 * inputs.ARCMIN, args.fit_order
+    P = (p_max + 1) * (p_max + 2) // 2
+    gen = torch.Generator("cuda:0").manual_seed(inputs.SEED_BASE + 40)
+    ax = (torch.arange(n, device="cuda:0", dtype=torch.float64) - (n - 1) / 2) * pix
+    L, M = -ax[None, :], ax[:, None]
+    img = torch.zeros((n, n), dtype=torch.float64, device="cuda:0")
+    cen = (torch.rand((40, 2), generator=gen, device="cuda:0", dtype=torch.float64) - 0.5) * 0.5 * n * pix
+    wid = (0.02 + 0.08 * torch.rand(40, generator=gen, device="cuda:0", dtype=torch.float64)) * n * pix
+    amp = torch.randn(40, generator=gen, device="cuda:0", dtype=torch.float64)
+    for k in range(40):
+        img += amp[k] * torch.exp(-((L - cen[k, 0]) ** 2 + (M - cen[k, 1]) ** 2) / (2 * wid[k] ** 2))
+    beta = 0.9 * n * pix * 2.3548 / (2.0 * 2.6 * (2 * p_max + 1.0) ** 0.5)
+    f1, f2 = np.meshgrid([0.9, 1.0, 1.1], [0.9, 1.0, 1.1], indexing="ij")
+    B1, B2 = (beta * f1).ravel(), (beta * f2).ravel()
+    beam = (3.0 * pix, 2.0 * pix, 0.5, 6)
+    call = lambda: ctx.fit_shapelets(img, -pix, pix, 0.0, 0.0, 0.0, 0.0, 0.3, p_max, B1, B2, beam=beam, want_weights=True)
+    for _ in range(max(1, args.warmup)):
+        out = call()
+    torch.cuda.synchronize()
+    ts, gs = [], []
+    l0 = binding.kernel_launches()
+    for _ in range(max(3, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); out = call(); e1.record(); torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1)); gs.append(ctx.fit_gram_ms())
+    launches = binding.kernel_launches() - l0
+    ctx.check()
+    coeff, resid, weights, best = out
+    ms, gram_ms = float(np.median(ts)), float(np.median(gs))
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = peaks.get("bf16_tflops", 1650.0)
+    n_pix = n * n
+    alg_flops = float(n_pix) * P * (P + 1)                      # A^T A, symmetric half, 2 flops per MAC
+    n_rt = (P + 127) // 128
+    exe_flops = 3.0 * 2.0 * (n_rt * (n_rt + 1) // 2) * 128 * 128 * ((n_pix + 63) // 64 * 64)
+    print(json.dumps({"fit": {
+        "workload": f"{n} x {n} pixel synthetic image, p_max {p_max} ({P} basis functions), 3 x 3 (beta1, beta2) grid, "
+                    f"beam stencil {2 * beam[3] + 1}^2, 6 refinement passes",
+        "ms_per_call": ms, "fits_per_s": 9.0 / (ms * 1e-3), "gpu_launches": launches, "best_index": int(best[0]),
+        "residual_best_over_image_power": float(resid[int(best[0])] / (img ** 2).sum()),
+        "roofline": {"bound": "tensor", "kernel": "fit_gram_kernel (tcgen05 kind::f16, FP16 hi+lo split, 3 products)",
+                     "achieved": alg_flops / (gram_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                     "frac": alg_flops / (gram_ms * 1e-3) / 1e12 / peak,
+                     "executed_tensor_tflops": exe_flops / (gram_ms * 1e-3) / 1e12,
+                     "ms_per_launch": gram_ms,
+                     "peak_source": ("MEASURED_PEAKS.json bf16_tflops (fp16 dense peak = bf16 dense peak nominally)"
+                                     if peaks else "fallback 1650 TFLOP/s"),
+                     "algorithmic_flops_per_launch": alg_flops,
+                     "note": "algorithmic = n_pix P (P + 1): the symmetric half of A^T A once; the kernel executes 3 "
+                             "split-precision products on 128-padded tiles (executed_tensor_tflops)", "traffic": None}}}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -694,6 +762,10 @@ def main():
                     help="look-up-table vs recurrence evaluation of the shapelet basis (PAPER.md:159) and exit")
     ap.add_argument("--peel", action="store_true",
                     help="time the gain fit and peel of PAPER.md section 5.1 on the config and exit")
+    ap.add_argument("--fit", action="store_true",
+                    help="time the image-space shapelet fit (PAPER.md section 2.1) on a synthetic image and exit")
+    ap.add_argument("--fit-pixels", type=int, default=256)
+    ap.add_argument("--fit-order", type=int, default=40)
     ap.add_argument("--truncation", action="store_true",
                     help="GPU time vs kept fraction of components (PAPER.md section 5.3) and exit")
     args = ap.parse_args()
@@ -710,6 +782,8 @@ def main():
         return run_basis(args)
     if args.peel:
         return run_peel(args)
+    if args.fit:
+        return run_fit(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

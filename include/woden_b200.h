@@ -267,6 +267,11 @@ int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const doub
                         const woden_restoring_beam *beam, int n_refine,
                         double *coeff, double *residual, double *weights, int *best, void *cuda_stream);
 
+/* Measurement aid: device time in milliseconds of the Gram-matrix kernel (the tcgen05 contraction) of
+ * the LAST (beta1, beta2) pair of the last woden_fit_shapelets call on this context, from CUDA events
+ * recorded around it on the call's stream.  Synchronises on that kernel.  WODEN_ERR_DIM before any fit. */
+int woden_fit_gram_ms(woden_ctx *ctx, float *ms);
+
 /* Basis-evaluation experiment: the 1-D shapelet series
  *   out[i] = sum_{p <= p_max} coeff[p] h_p(x[i]),   h_p(x) = H_p(x) exp(-x^2/2)/sqrt(2^p p!)
  * by the FP32 three-term recurrence of the predict kernels (WODEN_BASIS_RECURRENCE) or by the

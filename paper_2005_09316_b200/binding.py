@@ -40,7 +40,7 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -115,6 +115,7 @@ def load() -> C.CDLL:
                                       C.POINTER(woden_points_host), C.POINTER(woden_gaussians_host),
                                       C.POINTER(woden_shapelets_host), _vp, _vp]
     L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
+    L.woden_fit_gram_ms.argtypes = [_vp, C.POINTER(C.c_float)]
     L.woden_fit_shapelets.argtypes = [_vp, C.POINTER(woden_image_grid), _vp, C.c_double, C.c_double, C.c_double, C.c_int,
                                       C.c_int, _dp, _dp, C.POINTER(woden_restoring_beam), C.c_int, _vp, _vp, _vp, _vp, _vp]
     L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
@@ -369,6 +370,11 @@ class Woden:
                                          _stream_handle(stream))
         self._ck(rc, "woden_fit_shapelets")
         return coeff, resid, weights, best
+
+    def fit_gram_ms(self) -> float:
+        ms = C.c_float(0.0)
+        self._ck(self._L.woden_fit_gram_ms(self._ctx, C.byref(ms)), "woden_fit_gram_ms")
+        return float(ms.value)
 
     def pipe_rate(self, which: str, iters: int = 20000):
         ops, clk = C.c_double(0.0), C.c_double(0.0)

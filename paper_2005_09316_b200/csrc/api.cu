@@ -50,6 +50,7 @@ struct woden_ctx {
     std::vector<double> chan_s_host;     // nu_f / c of the padded channel list (host copy)
     cudaStream_t walk_stream = nullptr;  // second lane of the channel-walking launches
     cudaEvent_t walk_fork = nullptr, walk_join = nullptr;
+    cudaEvent_t fit_t0 = nullptr, fit_t1 = nullptr;   // around the last fit's Gram kernel
     int chan_F_pad = 0;
     ChanTable ch{};
     // woden_simulate_host staging
@@ -231,6 +232,7 @@ int woden_destroy(woden_ctx *ctx)
             cudaEventDestroy(ctx->walk_fork);
             cudaEventDestroy(ctx->walk_join);
         }
+        if (ctx->fit_t0) { cudaEventDestroy(ctx->fit_t0); cudaEventDestroy(ctx->fit_t1); }
         if (ctx->copy_stream) {
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
@@ -701,6 +703,11 @@ int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const doub
     w.ops = static_cast<__half *>(ctx->f_ops.p);
     w.partial = static_cast<float *>(ctx->f_part.p);
     w.err = static_cast<unsigned int *>(ctx->err.p);
+    if (!ctx->fit_t0) {
+        CU(ctx, cudaEventCreate(&ctx->fit_t0), "create event");
+        CU(ctx, cudaEventCreate(&ctx->fit_t1), "create event");
+    }
+    w.gram_t0 = ctx->fit_t0; w.gram_t1 = ctx->fit_t1;
     FitProblem f;
     f.n_l = grid->n_l; f.n_m = grid->n_m; f.p_max = p_max;
     f.half_width = has_beam ? beam->half_width : 0;
@@ -716,6 +723,17 @@ int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const doub
         CU(ctx, launch_fit_one(f, w, st), "fit launch");
     }
     if (best) CU(ctx, launch_fit_argmin(residual, n_beta, best, st), "fit argmin launch");
+    return WODEN_OK;
+}
+
+int woden_fit_gram_ms(woden_ctx *ctx, float *ms)
+{
+    if (!ctx || !ms) return WODEN_ERR_NULL;
+    if (!ctx->fit_t0) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    CU(ctx, cudaEventSynchronize(ctx->fit_t1), "fit timing sync");
+    CU(ctx, cudaEventElapsedTime(ms, ctx->fit_t0, ctx->fit_t1), "fit timing");
     return WODEN_OK;
 }
 

@@ -549,7 +549,9 @@ cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_
     const int gsmem = GSTAGES * G_STAGE_BYTES;
     cudaError_t e = cudaFuncSetAttribute(fit_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, gsmem);
     if (e != cudaSuccess) return e;
+    if (w.gram_t0) cudaEventRecord(w.gram_t0, st);
     fit_gram_kernel<<<dim3(sz.n_pairs, sz.n_split), 128, gsmem, st>>>(gp); note_launch();
+    if (w.gram_t1) cudaEventRecord(w.gram_t1, st);
     // relative diagonal loading: the split-FP16 Gram matrix carries ~2^-21 sqrt(G_rr G_cc) of error per
     // entry; loading the diagonal by 2^-14 keeps the preconditioner positive definite for ~10^3 unknowns
     const double ridge = ldexp(1.0, -14);

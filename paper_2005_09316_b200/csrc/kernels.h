@@ -113,6 +113,7 @@ struct FitScratch {
     __half *ops;
     float *partial;
     unsigned int *err;
+    cudaEvent_t gram_t0, gram_t1;        // recorded around the Gram kernel when not NULL (bench.py --fit)
 };
 cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st);
 cudaError_t launch_fit_argmin(const double *residual, int n, int *best, cudaStream_t st);
