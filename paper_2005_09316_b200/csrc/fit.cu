@@ -109,31 +109,43 @@ __global__ void fit_stencil_kernel(double dl, double dm, double bmaj, double bmi
     for (int k = threadIdx.x; k < n; k += blockDim.x) stencil[k] *= inv;
 }
 
-// out[q][t][s] = sum_{dt, ds} stencil[dt][ds] in[q][t - dt][s - ds], zero outside the image.
-// One CTA = one basis image row-block of 16 x 16 output pixels; the stencil is centro-symmetric, so
-// correlation and convolution coincide.
-__global__ void fit_convolve_kernel(const double *__restrict__ in, const double *__restrict__ stencil, int n_l, int n_m,
-                                    int hw, double *__restrict__ out)
+// out[q][t][s] = sum_{dt, ds} stencil[dt][ds] in[q][t - (dt - hw)][s - (ds - hw)], zero outside the image.
+// One CTA = 64 x 16 output pixels of one basis image; a thread owns 4 consecutive pixels along s and
+// slides a 4-value register window over the shared-memory patch (one patch load per 4 FMAs).
+constexpr int CV_W = 64, CV_H = 16;
+__global__ void __launch_bounds__(256) fit_convolve_kernel(const double *__restrict__ in, const double *__restrict__ stencil,
+                                                           int n_l, int n_m, int hw, double *__restrict__ out)
 {
     extern __shared__ double sm[];
-    const int w = 2 * hw + 1, tile = 16 + 2 * hw;
+    const int w = 2 * hw + 1, tw = CV_W + 2 * hw, th = CV_H + 2 * hw;
     double *st = sm, *patch = sm + w * w;
-    const int q = blockIdx.z, s0 = blockIdx.x * 16, t0 = blockIdx.y * 16;
+    const int q = blockIdx.z, s0 = blockIdx.x * CV_W, t0 = blockIdx.y * CV_H;
     const double *img = in + (size_t)q * n_l * n_m;
-    const int tid = threadIdx.y * 16 + threadIdx.x;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * 16 + tx;
     for (int k = tid; k < w * w; k += 256) st[k] = stencil[k];
-    for (int k = tid; k < tile * tile; k += 256) {
-        const int s = s0 - hw + k % tile, t = t0 - hw + k / tile;
+    for (int k = tid; k < tw * th; k += 256) {
+        const int s = s0 - hw + k % tw, t = t0 - hw + k / tw;
         patch[k] = (s >= 0 && s < n_l && t >= 0 && t < n_m) ? img[(size_t)t * n_l + s] : 0.0;
     }
     __syncthreads();
-    const int s = s0 + threadIdx.x, t = t0 + threadIdx.y;
-    if (s >= n_l || t >= n_m) return;
-    double acc = 0.0;
-    for (int dt = 0; dt < w; ++dt)
-        for (int ds = 0; ds < w; ++ds)
-            acc = fma(st[dt * w + ds], patch[(threadIdx.y + 2 * hw - dt) * tile + threadIdx.x + 2 * hw - ds], acc);
-    out[(size_t)q * n_l * n_m + (size_t)t * n_l + s] = acc;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int dt = 0; dt < w; ++dt) {
+        const double *row = patch + (ty + 2 * hw - dt) * tw + 4 * tx + 2 * hw;      // ds = 0 position of output 0
+        double v1 = row[1], v2 = row[2], v3 = row[3];
+        for (int ds = 0; ds < w; ++ds) {
+            const double v0 = row[-ds], c = st[dt * w + ds];
+            acc[0] = fma(c, v0, acc[0]); acc[1] = fma(c, v1, acc[1]);
+            acc[2] = fma(c, v2, acc[2]); acc[3] = fma(c, v3, acc[3]);
+            v3 = v2; v2 = v1; v1 = v0;
+        }
+    }
+    const int t = t0 + ty;
+    if (t >= n_m) return;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int s = s0 + 4 * tx + i;
+        if (s < n_l) out[(size_t)q * n_l * n_m + (size_t)t * n_l + s] = acc[i];
+    }
 }
 
 // ---------------------------------------------------------------------------------- 3. scaling
@@ -312,37 +324,122 @@ __global__ void fit_gram_reduce_kernel(const float *__restrict__ partial, int n_
 }
 
 // ---------------------------------------------------------------------------------- 5. solve
-// In-place Cholesky G = L L^T by one CTA: on return the lower triangle holds L and the upper triangle
-// L^T (so that both triangular solves read rows).  Left-looking, one warp per row of the column.
-__global__ void __launch_bounds__(1024) fit_cholesky_kernel(double *__restrict__ G, int n, unsigned int *__restrict__ err)
+// In-place blocked Cholesky G = L L^T (right-looking, panels of CB = 64 columns; n is a multiple of
+// 128): per panel three kernels -- the 64 x 64 diagonal block in shared memory by one CTA, the rows
+// below it by triangular solves (one CTA per 64 rows), then the rank-64 update of the trailing lower
+// triangle (one CTA per 64 x 64 tile).  On return the lower triangle holds L and the upper triangle
+// L^T, so that both triangular solves of the refinement read rows.
+constexpr int CB = 64;
+
+__global__ void __launch_bounds__(256) chol_diag_kernel(double *__restrict__ G, int n, int j0, unsigned int *__restrict__ err)
 {
-    __shared__ double col_s[FIT_MAX_N];                          // s_i of the current column, i >= j
-    __shared__ double piv;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
-    for (int j = 0; j < n; ++j) {
-        const double *Lj = G + (size_t)j * n;
-        // s_i = G[i][j] - sum_{k<j} L[i][k] L[j][k] for i >= j
-        for (int i = j + warp; i < n; i += n_warps) {
-            const double *Li = G + (size_t)i * n;
-            double s = 0.0;
-            for (int k = lane; k < j; k += 32) s = fma(Li[k], Lj[k], s);
-            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            if (lane == 0) col_s[i - j] = Li[j] - s;
+    __shared__ double D[CB][CB + 1];
+    const int tid = threadIdx.x;
+    for (int e = tid; e < CB * CB; e += 256) {
+        const int r = e / CB, c = e % CB;
+        D[r][c] = c <= r ? G[(size_t)(j0 + r) * n + j0 + c] : 0.0;
+    }
+    __syncthreads();
+    for (int c = 0; c < CB; ++c) {
+        if (tid == 0) {
+            double d = D[c][c];
+            if (!(d > 0.0)) { atomicAdd(err, 1u); d = 1.0; }      // not positive definite: counted (woden_check)
+            D[c][c] = sqrt(d);
         }
         __syncthreads();
-        if (threadIdx.x == 0) {
-            double d = col_s[0];
-            if (!(d > 0.0)) { atomicAdd(err, 1u); d = 1.0; }      // not positive definite: counted (woden_check), kept finite
-            piv = sqrt(d);
+        if (tid > c && tid < CB) D[tid][c] /= D[c][c];
+        __syncthreads();
+        // trailing update of the block's lower triangle: D[r][k] -= D[r][c] D[k][c], c < k <= r
+        for (int e = tid; e < CB * CB; e += 256) {
+            const int r = e / CB, k = e % CB;
+            if (k > c && k <= r) D[r][k] = fma(-D[r][c], D[k][c], D[r][k]);
         }
         __syncthreads();
-        const double inv = 1.0 / piv;
-        for (int i = j + threadIdx.x; i < n; i += blockDim.x) {
-            const double v = (i == j) ? piv : col_s[i - j] * inv;
-            G[(size_t)i * n + j] = v;
-            G[(size_t)j * n + i] = v;
+    }
+    for (int e = tid; e < CB * CB; e += 256) {
+        const int r = e / CB, c = e % CB;
+        if (c <= r) {
+            G[(size_t)(j0 + r) * n + j0 + c] = D[r][c];
+            G[(size_t)(j0 + c) * n + j0 + r] = D[r][c];
         }
-        __syncthreads();
+    }
+}
+
+// rows below the diagonal block: X L_d^T = A  (thread = one row, forward substitution over 64 columns)
+__global__ void __launch_bounds__(CB) chol_trsm_kernel(double *__restrict__ G, int n, int j0)
+{
+    extern __shared__ double chol_sm[];
+    double (*Ld)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(chol_sm);
+    double (*X)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(chol_sm + CB * (CB + 1));
+    const int tid = threadIdx.x, r0 = j0 + CB + blockIdx.x * CB;
+    for (int e = tid; e < CB * CB; e += CB) {
+        const int r = e / CB, c = e % CB;
+        Ld[r][c] = G[(size_t)(j0 + r) * n + j0 + c];
+        X[r][c] = G[(size_t)(r0 + r) * n + j0 + c];               // coalesced over c
+    }
+    __syncthreads();
+    for (int c = 0; c < CB; ++c) {
+        double s = X[tid][c];
+        for (int k = 0; k < c; ++k) s = fma(-X[tid][k], Ld[c][k], s);
+        X[tid][c] = s / Ld[c][c];
+    }
+    __syncthreads();
+    for (int e = tid; e < CB * CB; e += CB) {
+        const int r = e / CB, c = e % CB;
+        G[(size_t)(r0 + r) * n + j0 + c] = X[r][c];
+    }
+    for (int e = tid; e < CB * CB; e += CB) {
+        const int c = e / CB, r = e % CB;                         // coalesced over r: the mirrored copy
+        G[(size_t)(j0 + c) * n + r0 + r] = X[r][c];
+    }
+}
+
+// trailing lower triangle: G[bi][bj] -= X_bi X_bj^T for the 64 x 64 tiles bj <= bi below the panel
+__global__ void __launch_bounds__(256) chol_syrk_kernel(double *__restrict__ G, int n, int j0)
+{
+    extern __shared__ double chol_sm[];
+    double (*Xi)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(chol_sm);
+    double (*Xj)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(chol_sm + CB * (CB + 1));
+    int bi = 0, rem = blockIdx.x;
+    while (rem > bi) { rem -= bi + 1; ++bi; }
+    const int bj = rem;
+    const int ri = j0 + CB + bi * CB, rj = j0 + CB + bj * CB;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < CB * CB; e += 256) {
+        const int r = e / CB, c = e % CB;
+        Xi[r][c] = G[(size_t)(ri + r) * n + j0 + c];
+        Xj[r][c] = G[(size_t)(rj + r) * n + j0 + c];
+    }
+    __syncthreads();
+    const int tr = (tid / 16) * 4, tc = (tid % 16) * 4;
+    double acc[4][4] = {};
+    for (int k = 0; k < CB; ++k) {
+        double a[4], b[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { a[i] = Xi[tr + i][k]; b[i] = Xj[tc + i][k]; }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) G[(size_t)(ri + tr + i) * n + rj + tc + j] -= acc[i][j];
+}
+
+void launch_cholesky(double *G, int n, unsigned int *err, cudaStream_t st)
+{
+    constexpr int SM2 = 2 * CB * (CB + 1) * (int)sizeof(double);
+    cudaFuncSetAttribute(chol_trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SM2);
+    cudaFuncSetAttribute(chol_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SM2);
+    for (int j0 = 0; j0 < n; j0 += CB) {
+        chol_diag_kernel<<<1, 256, 0, st>>>(G, n, j0, err); note_launch();
+        const int below = (n - j0 - CB) / CB;
+        if (below > 0) {
+            chol_trsm_kernel<<<below, CB, SM2, st>>>(G, n, j0); note_launch();
+            chol_syrk_kernel<<<below * (below + 1) / 2, 256, SM2, st>>>(G, n, j0); note_launch();
+        }
     }
 }
 
@@ -352,7 +449,7 @@ __global__ void __launch_bounds__(1024) fit_cholesky_kernel(double *__restrict__
 __global__ void __launch_bounds__(1024) fit_solve_kernel(const double *__restrict__ G, int n, const double *__restrict__ g,
                                                          double *__restrict__ z)
 {
-    __shared__ double y[FIT_MAX_N], part[32];
+    __shared__ double y[FIT_MAX_N], part[32], Dg[32][33];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = g[i];
     __syncthreads();
@@ -362,19 +459,26 @@ __global__ void __launch_bounds__(1024) fit_solve_kernel(const double *__restric
         if (i < n) {
             const double *Li = G + (size_t)i * n;
             double s = 0.0;
-            for (int k = lane; k < r0; k += 32) s = fma(Li[k], y[k], s);
+            double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            int k = lane;
+            for (; k + 96 < r0; k += 128) {                       // four loads in flight per lane
+                s = fma(Li[k], y[k], s); s1 = fma(Li[k + 32], y[k + 32], s1);
+                s2 = fma(Li[k + 64], y[k + 64], s2); s3 = fma(Li[k + 96], y[k + 96], s3);
+            }
+            for (; k < r0; k += 32) s = fma(Li[k], y[k], s);
+            s = (s + s1) + (s2 + s3);
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
             if (lane == 0) part[warp] = y[i] - s;
+            if (r0 + lane < n) Dg[warp][lane] = Li[r0 + lane];      // the 32 x 32 diagonal block (lower part used)
         }
         __syncthreads();
         if (warp == 0) {
             const int rows = min(32, n - r0);
             double v = lane < rows ? part[lane] : 0.0;
             for (int c = 0; c < rows; ++c) {
-                const double d = G[(size_t)(r0 + c) * n + r0 + c];
-                const double yc = __shfl_sync(0xffffffffu, v, c) / d;
+                const double yc = __shfl_sync(0xffffffffu, v, c) / Dg[c][c];
                 if (lane == c) v = yc;
-                else if (lane > c && lane < rows) v -= G[(size_t)(r0 + lane) * n + r0 + c] * yc;
+                else if (lane > c && lane < rows) v -= Dg[lane][c] * yc;
             }
             if (lane < rows) y[r0 + lane] = v;
         }
@@ -388,19 +492,26 @@ __global__ void __launch_bounds__(1024) fit_solve_kernel(const double *__restric
         if (i < r1) {
             const double *Ui = G + (size_t)i * n;
             double s = 0.0;
-            for (int k = r1 + lane; k < n; k += 32) s = fma(Ui[k], y[k], s);
+            double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            int k = r1 + lane;
+            for (; k + 96 < n; k += 128) {
+                s = fma(Ui[k], y[k], s); s1 = fma(Ui[k + 32], y[k + 32], s1);
+                s2 = fma(Ui[k + 64], y[k + 64], s2); s3 = fma(Ui[k + 96], y[k + 96], s3);
+            }
+            for (; k < n; k += 32) s = fma(Ui[k], y[k], s);
+            s = (s + s1) + (s2 + s3);
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
             if (lane == 0) part[warp] = y[i] - s;
+            if (r0 + lane < n) Dg[warp][lane] = Ui[r0 + lane];      // diagonal block of L^T (upper part used)
         }
         __syncthreads();
         if (warp == 0) {
             const int rows = r1 - r0;
             double v = lane < rows ? part[lane] : 0.0;
             for (int c = rows - 1; c >= 0; --c) {
-                const double d = G[(size_t)(r0 + c) * n + r0 + c];
-                const double xc = __shfl_sync(0xffffffffu, v, c) / d;
+                const double xc = __shfl_sync(0xffffffffu, v, c) / Dg[c][c];
                 if (lane == c) v = xc;
-                else if (lane < c) v -= G[(size_t)(r0 + lane) * n + r0 + c] * xc;
+                else if (lane < c) v -= Dg[lane][c] * xc;
             }
             if (lane < rows) y[r0 + lane] = v;
         }
@@ -530,12 +641,12 @@ cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_
     fit_product_kernel<<<dim3((n_pix + 255) / 256, P), 256, 0, st>>>(w.hx, w.hx + (size_t)(f.p_max + 1) * n_pix, n_pix,
                                                                       f.p_max, P, norm, unconv); note_launch();
     if (beam) {
-        const int hw = f.half_width, wd = 2 * hw + 1, tile = 16 + 2 * hw;
-        const size_t smem = ((size_t)wd * wd + (size_t)tile * tile) * sizeof(double);
+        const int hw = f.half_width, wd = 2 * hw + 1;
+        const size_t smem = ((size_t)wd * wd + (size_t)(CV_W + 2 * hw) * (CV_H + 2 * hw)) * sizeof(double);
         cudaError_t e = cudaFuncSetAttribute(fit_convolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         fit_stencil_kernel<<<1, 256, 0, st>>>(f.dl, f.dm, f.bmaj, f.bmin, sin(f.bpa), cos(f.bpa), hw, w.stencil); note_launch();
-        fit_convolve_kernel<<<dim3((f.n_l + 15) / 16, (f.n_m + 15) / 16, P), dim3(16, 16), smem, st>>>(w.a0, w.stencil, f.n_l,
+        fit_convolve_kernel<<<dim3((f.n_l + CV_W - 1) / CV_W, (f.n_m + CV_H - 1) / CV_H, P), dim3(16, 16), smem, st>>>(w.a0, w.stencil, f.n_l,
                                                                                                       f.n_m, hw, w.at); note_launch();
     }
     fit_scale_rows_kernel<<<P, 256, 0, st>>>(w.at, n_pix, w.scale, w.abssum); note_launch();
@@ -557,7 +668,7 @@ cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_
     const double ridge = ldexp(1.0, -14);
     fit_gram_reduce_kernel<<<dim3((sz.n_pad + 127) / 128, sz.n_pad), 128, 0, st>>>(w.partial, sz.n_split, sz.n_pairs, sz.n_rt,
                                                                                   P, ridge, w.gram); note_launch();
-    fit_cholesky_kernel<<<1, 1024, 0, st>>>(w.gram, sz.n_pad, w.err); note_launch();
+    launch_cholesky(w.gram, sz.n_pad, w.err, st);
     fit_zero_kernel<<<(sz.n_pad + 255) / 256, 256, 0, st>>>(w.z, sz.n_pad); note_launch();
     for (int it = 0; it <= f.n_refine; ++it) {
         fit_residual_kernel<<<(n_pix + 127) / 128, 128, P * sizeof(double), st>>>(w.at, w.z, f.image, P, n_pix, w.r); note_launch();
