@@ -254,7 +254,7 @@ def run_ours(args):
     wl = parallel.rank_workload(args.config, rank, world, scaling="weak")
     ctx = binding.Woden(local)
     ctx.set_path(binding.WODEN_PATH_GENERAL if args.path == "general" else binding.WODEN_PATH_AUTO)
-    dw = binding.DeviceWorkload(wl, device=f"cuda:{local}")
+    dw = binding.DeviceWorkload(wl, device=f"cuda:{local}", ctx=ctx)
     vis = ctx.new_vis(dw.uvw)
     counts = workload_counts(wl)
     comps = wl.points.n + wl.gaussians.n + wl.shapelets.n

@@ -189,8 +189,13 @@ def predict_workload(wl, vis_index=None) -> np.ndarray:
                           wl.ref_freq_hz, g.maj_fwhm_rad, g.min_fwhm_rad, g.pa_rad,
                           vis_index=vis_index, out=out, accumulate=True)
     if s.n:
+        # M_j (reading G4) from the oracle's own routine, not from the generator's arrays: the CUDA side
+        # computes its own too (woden_shapelet_uv_basis), so the two sides share only l, m and dec0
+        M = s.uv_basis
+        if M is not None and "dec0_rad" in wl.meta:
+            M = shapelet_uv_basis(s.l, s.m, wl.meta["dec0_rad"])
         predict_shapelets(wl.u_m, wl.v_m, wl.w_m, wl.freqs_hz, s.l, s.m, s.s0_jy, s.alpha,
-                          wl.ref_freq_hz, s.beta1_rad, s.beta2_rad, s.pa_rad, s.uv_basis,
+                          wl.ref_freq_hz, s.beta1_rad, s.beta2_rad, s.pa_rad, M,
                           s.coeff_offset, s.n1, s.n2, s.coeff,
                           vis_index=vis_index, out=out, accumulate=True)
     return out

@@ -389,9 +389,12 @@ def kernel_launches() -> int:
 
 
 class DeviceWorkload:
-    """A generated Workload copied to the GPU once (device-resident inputs for the C-ABI calls)."""
+    """A generated Workload copied to the GPU once (device-resident inputs for the C-ABI calls).
+    With `ctx`, the shapelets' M_j (reading G4) are computed by the library itself
+    (woden_shapelet_uv_basis from l, m and the phase-centre declination in wl.meta) instead of being
+    copied from the generator's arrays."""
 
-    def __init__(self, wl, device="cuda:0"):
+    def __init__(self, wl, device="cuda:0", ctx=None):
         import torch
 
         def t(a, dtype=torch.float64):
@@ -405,8 +408,11 @@ class DeviceWorkload:
         self.g = (t(g.l), t(g.m), t(g.s0_jy), t(g.alpha), t(g.maj_fwhm_rad), t(g.min_fwhm_rad),
                   t(g.pa_rad)) if g.n else None
         if s.n:
+            M = t(s.uv_basis)
+            if ctx is not None and s.uv_basis is not None and "dec0_rad" in wl.meta:
+                M = ctx.shapelet_uv_basis(t(s.l), t(s.m), wl.meta["dec0_rad"])
             self.s = (t(s.l), t(s.m), t(s.s0_jy), t(s.alpha), t(s.beta1_rad), t(s.beta2_rad), t(s.pa_rad),
-                      t(s.uv_basis), t(s.coeff_offset, torch.int32), int(s.coeff_offset[-1]),
+                      M, t(s.coeff_offset, torch.int32), int(s.coeff_offset[-1]),
                       int((s.n1 + s.n2).max()), t(s.n1, torch.int32), t(s.n2, torch.int32), t(s.coeff))
         else:
             self.s = None

@@ -46,6 +46,7 @@ CONFIG_NAMES = {
     4: "Fornax-A-like shapelet model",
     5: "Full-band mixed sky",
     6: "Phase-II-like shapelet model (extra: SURVEY.md 8(f) NEXT-2)",
+    7: "Phase-II-like point / Gaussian sky (extra: parity case on 5.5 km baselines)",
 }
 
 
@@ -253,6 +254,9 @@ _OBS = {  # config: (array, T, dt_s, F)
     # not a BASELINE.json config: the 5.5 km phase II-like array with the paper's p_max = 86 lobes
     # (PAPER.md:171, :183), the sixth case SURVEY.md 8(f) NEXT-2 suggests
     6: ("A128L", 14, 8.0, 384),
+    # not a BASELINE.json config: points and Gaussians on the same 5.5 km array, where the phase budget
+    # of the channel-walking path is tightest; a parity case only
+    7: ("A128L", 4, 8.0, 96),
 }
 
 
@@ -262,7 +266,7 @@ def make_antennas(config: int, *, t_index0: int = 0, n_times_total: Optional[int
     (X, Y, Z) in metres [n_ant], hour angles [T] in radians, and the phase-centre declination --
     the inputs of woden_uvw_from_antennas.  Same draws as make_config."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..6, got {config}")
+        raise ValueError(f"config must be 1..7, got {config}")
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + config))
     arr, T, dt, _ = _OBS[config]
     if n_times is None:
@@ -279,7 +283,7 @@ def make_antennas(config: int, *, t_index0: int = 0, n_times_total: Optional[int
 def make_config_shape(config: int):
     """(array name, T, dt_s, F) of config 1..5 without generating it."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..6, got {config}")
+        raise ValueError(f"config must be 1..7, got {config}")
     return _OBS[config]
 
 
@@ -289,7 +293,7 @@ def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] 
     longer observation with the same sky and array (weak-scaling ranks, SURVEY.md §8(e));
     the defaults give the config exactly as BASELINE.json words it."""
     if config not in _OBS:
-        raise ValueError(f"config must be 1..6, got {config}")
+        raise ValueError(f"config must be 1..7, got {config}")
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + config))
     arr, T, dt, F = _OBS[config]
     if n_times is None:
@@ -331,6 +335,9 @@ def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] 
     elif config == 6:
         cl = np.array([-np.sin(np.deg2rad(0.25)), np.sin(np.deg2rad(0.25))])
         shp = _shapelets(rng, cl, np.zeros(2), 86, 5.0, 20.0)
+    elif config == 7:
+        pts = _points(rng, 1500, 25.0, 0.01, 10.0)
+        gau = _gaussians(rng, 700, 25.0, 0.01, 10.0, 0.5, 30.0)
     elif config == 5:
         pts = _points(rng, 8000, 25.0, 0.01, 10.0)
         gau = _gaussians(rng, 2000, 25.0, 0.01, 10.0, 1.0, 30.0)
@@ -340,7 +347,7 @@ def make_config(config: int, *, t_index0: int = 0, n_times_total: Optional[int] 
     return Workload(config=config, name=CONFIG_NAMES[config], u_m=u, v_m=v, w_m=w,
                     freqs_hz=freqs, ref_freq_hz=REF_FREQ_HZ, points=pts, gaussians=gau,
                     shapelets=shp,
-                    meta={"array": arr, "dt_s": dt, "t_index0": t_index0,
+                    meta={"array": arr, "dt_s": dt, "t_index0": t_index0, "dec0_rad": float(np.deg2rad(DEC0_DEG)),
                           "seed": SEED_BASE + config})
 
 

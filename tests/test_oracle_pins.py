@@ -411,6 +411,19 @@ def test_tolerance_scale_definition():
     ref += (np.abs(wl.gaussians.s0_jy) * fr ** wl.gaussians.alpha).sum(1)
     ref += (np.abs(wl.shapelets.s0_jy) * fr ** wl.shapelets.alpha).sum(1) * np.abs(wl.shapelets.coeff).sum()
     assert np.allclose(sc, ref, rtol=1e-13)
+    # signs: negative fluxes and negative coefficients enter by absolute value (hand-computed case:
+    # S = -2 and +3 at nu = ref, alpha irrelevant there; shapelet S = -1.5 with coefficients 1, -2, 0.5)
+    fr1 = np.array([wl.ref_freq_hz])
+    assert oracle.tolerance_scale(fr1, [-2.0, 3.0], [-0.7, 0.3], wl.ref_freq_hz)[0] == pytest.approx(5.0, rel=1e-15)
+    assert oracle.tolerance_scale(fr1, [-1.5], [-0.8], wl.ref_freq_hz, [0, 3], [1.0, -2.0, 0.5])[0] == pytest.approx(
+        5.25, rel=1e-15)
+    # and at another frequency the law is |s0| (nu/ref)^alpha, never negative
+    two = oracle.tolerance_scale(np.array([2.0 * wl.ref_freq_hz]), [-2.0], [-1.0], wl.ref_freq_hz)
+    assert two[0] == pytest.approx(1.0, rel=1e-15)
+    wl4 = inputs.make_config(4)                                   # 25 % negative components
+    sc4 = oracle.tolerance_scale(wl4.freqs_hz[:3], wl4.points.s0_jy, wl4.points.alpha, wl4.ref_freq_hz)
+    ref4 = (np.abs(wl4.points.s0_jy) * (wl4.freqs_hz[:3, None] / wl4.ref_freq_hz) ** wl4.points.alpha).sum(1)
+    assert (wl4.points.s0_jy < 0).any() and np.allclose(sc4, ref4, rtol=1e-13)
 
 
 # ----------------------------------------------------------------------------- P16 (NEXT-2)
