@@ -214,7 +214,8 @@ int woden_shapelet_uv_basis(woden_ctx *ctx, int n, const double *l, const double
  * each step is the minimum-norm least-squares solution).  vis_data (V) and vis_model (I): DEVICE
  * complex64 [n_cells][n_antennas (n_antennas - 1) / 2], i.e. a woden_predict_* buffer viewed as
  * n_cells = n_times * n_freqs cells of all pairs i < j in i-major order.  gains: DEVICE complex128
- * [n_cells][n_antennas], written.  n_antennas is limited by shared memory (<= 161).
+ * [n_cells][n_antennas], written.  n_antennas is limited by shared memory (the strict upper
+ * triangle of |I_ij|^2 in FP64 plus 12 vectors: <= 200).
  * The spline smoothing of the gains across the band (:237) is not implemented. */
 int woden_calibrate_gains(woden_ctx *ctx, int n_antennas, long long n_cells,
                           const float *vis_data, const float *vis_model, int n_iter,

@@ -629,7 +629,7 @@ int woden_calibrate_gains(woden_ctx *ctx, int n_antennas, long long n_cells, con
 {
     if (!ctx || !vis_data || !vis_model || !gains) return WODEN_ERR_NULL;
     if (n_antennas < 2 || n_cells <= 0 || n_cells > 2147483647LL || n_iter < 0) return WODEN_ERR_DIM;
-    if (calibrate_smem_bytes(n_antennas) > 227u * 1024u) return WODEN_ERR_DIM;     // W must fit shared memory
+    if (n_antennas > 200 || calibrate_smem_bytes(n_antennas) > 227u * 1024u) return WODEN_ERR_DIM;   // W must fit shared memory
     Bind bind(ctx);
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

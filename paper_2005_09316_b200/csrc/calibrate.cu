@@ -10,12 +10,11 @@
 //   q_i = |g_i|^2,  d_i = sum_j W_ij q_j,  rho_i = [ sum_j g_j conj(I_ij) V_ij  -  g_i d_i ] / g_i
 //   (Q D + Q W Q) Re eps = q o Re rho          symmetric positive definite
 //   (Q D - Q W Q) Im eps = q o Im rho          symmetric, null vector (1,..,1): the overall phase
-// (I_ji = conj I_ij, V_ji = conj V_ij).  One CTA per cell keeps W in shared memory (FP64, N x N) and
-// solves both systems together by Jacobi-preconditioned conjugate gradients; the singular one is
+// (I_ji = conj I_ij, V_ji = conj V_ij).  One CTA per cell keeps W in shared memory (FP64, upper triangle)
+// and solves both systems together by Jacobi-preconditioned conjugate gradients; the singular one is
 // started from zero with its right-hand side projected on the range, and the result is moved to
 // the minimum-norm solution in e (the one Eq 22 has as a pseudo-inverse; reading G16) by removing
-// the component along the gauge direction i g.  All FP64.  Matrix-vector products read W[j][i]
-// (symmetric) so that a warp's lanes touch consecutive shared-memory words.
+// the component along the gauge direction i g.  All FP64.
 #include <cmath>
 
 #include "kernels.h"
@@ -23,7 +22,7 @@
 namespace woden {
 namespace {
 
-constexpr int CAL_THREADS = 512;
+constexpr int CAL_THREADS = 256;
 
 struct CalParams {
     const float2 *data, *model;   // [cells][B] complex64
@@ -47,61 +46,68 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// sum of up to four per-thread values over the CTA; every thread gets the totals
+// sum of up to NV per-thread values over the CTA; every thread gets the totals.  One barrier per call:
+// consecutive calls alternate between two scratch areas (`flip`), so a slow thread still reading the
+// totals of call n cannot be overtaken by the partial sums of call n + 1.
 template <int NV>
-__device__ __forceinline__ void block_sum(double (&v)[NV], double *scratch /* [NV][CAL_THREADS / 32] */)
+__device__ __forceinline__ void block_sum(double (&v)[NV], double *scratch /* [2][NV_MAX][CAL_THREADS / 32] */, int &flip)
 {
+    constexpr int NW = CAL_THREADS / 32, NV_MAX = 5;
+    static_assert(NV <= NV_MAX, "scratch size");
+    double *sc = scratch + flip * NV_MAX * NW;
+    flip ^= 1;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
         const double s = warp_sum(v[k]);
-        if (lane == 0) scratch[k * (CAL_THREADS / 32) + wid] = s;
+        if (lane == 0) sc[k * NW + wid] = s;
     }
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
         double s = 0.0;
 #pragma unroll
-        for (int w = 0; w < CAL_THREADS / 32; ++w) s += scratch[k * (CAL_THREADS / 32) + w];
+        for (int w = 0; w < NW; ++w) s += sc[k * NW + w];
         v[k] = s;
     }
-    __syncthreads();
 }
 
-__global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams p)
+// One CTA per (time, frequency) cell.  W_ij = |I_ij|^2 is kept in shared memory as its strict upper
+// triangle in the visibilities' own pair order (FP64, N (N - 1) / 2 words: 65 KB for 128 antennas, so two
+// cells are resident per SM and one cell's barrier waits are covered by the other's arithmetic).
+// Both systems are solved together by Jacobi-preconditioned conjugate gradients in the
+// single-reduction form (Chronopoulos & Gear): per iteration one matrix-vector product and ONE fused
+// reduction (gamma = (r, u), delta = (A u, u)), three barriers in all.
+__global__ void __launch_bounds__(CAL_THREADS, 2) calibrate_kernel(const CalParams p)
 {
     extern __shared__ __align__(16) double sm[];
     const int N = p.N, tid = threadIdx.x;
-    double *W = sm;                              // [N][N]
-    double *q = W + (size_t)N * N;               // |g|^2
+    double *Wt = sm;                             // [N (N - 1) / 2] strict upper triangle, pair order
+    double2 *qu = reinterpret_cast<double2 *>(Wt + p.B + (p.B & 1));   // q o (u0, u1); even offset: 16-byte aligned
+    double *q = reinterpret_cast<double *>(qu + N);  // |g|^2
     double *d = q + N;                           // sum_j W_ij q_j
     double *gre = d + N, *gim = gre + N;         // gains
     double *rhs0 = gim + N, *rhs1 = rhs0 + N;    // q o Re rho, q o Im rho
-    double *x0 = rhs1 + N, *x1 = x0 + N;         // CG iterates (Re eps, Im eps)
-    double *r0 = x1 + N, *r1 = r0 + N;           // CG residuals
-    double *p0 = r1 + N, *p1 = p0 + N;           // CG directions (pre-multiplied by q for the product)
-    double *a0 = p1 + N, *a1 = a0 + N;           // M p
-    double *scratch = a1 + N;                    // [4][CAL_THREADS / 32]
-    double *part = scratch + 4 * (CAL_THREADS / 32);   // [split][2][N] partial products, split N <= CAL_THREADS
-    double *invd = part + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS);    // Jacobi preconditioner 1 / (q d)
-    double2 *qp = reinterpret_cast<double2 *>(invd + N);   // q o (p0, p1); offset N (N + 15) + 4 (CAL_THREADS / 32) + 2 max(N, CAL_THREADS) doubles is even: 16-byte aligned
+    double *x1s = rhs1 + N;                      // Im eps (for the gauge step)
+    double *scratch = x1s + N;                   // [2][5][CAL_THREADS / 32]
+    double *part = scratch + 10 * (CAL_THREADS / 32);   // [split][2][N] partial products, split N <= CAL_THREADS
+    int *rowoff = reinterpret_cast<int *>(part + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS));   // pair(i, j) = rowoff[i] + j, i < j
     const int split = N >= CAL_THREADS ? 1 : CAL_THREADS / N;
     const int jchunk = (N + split - 1) / split;
+    int flip = 0;
 
     const float2 *V = p.data + (size_t)blockIdx.x * p.B;
     const float2 *I = p.model + (size_t)blockIdx.x * p.B;
 
-    // W_ij = |I_ij|^2 (FP64 from the complex64 model), symmetric, zero diagonal
-    for (int idx = tid; idx < N * N; idx += CAL_THREADS) {
-        const int i = idx / N, j = idx - i * N;
-        double w = 0.0;
-        if (i != j) {
-            const float2 m = I[i < j ? pair_index(i, j, N) : pair_index(j, i, N)];
-            w = (double)m.x * m.x + (double)m.y * m.y;
-        }
-        W[idx] = w;
+    // W = |I|^2 (FP64 from the complex64 model), coalesced over the pair list
+    for (long long b = tid; b < p.B; b += CAL_THREADS) {
+        const float2 m = I[b];
+        Wt[b] = (double)m.x * m.x + (double)m.y * m.y;
     }
-    for (int i = tid; i < N; i += CAL_THREADS) { gre[i] = 1.0; gim[i] = 0.0; }
+    for (int i = tid; i < N; i += CAL_THREADS) {
+        gre[i] = 1.0; gim[i] = 0.0;
+        rowoff[i] = (int)((long long)i * (2 * N - i - 1) / 2) - i - 1;
+    }
     __syncthreads();
 
     for (int it = 0; it < p.n_iter; ++it) {
@@ -113,8 +119,8 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
 #pragma unroll 4
             for (int j = tid & 31; j < N; j += 32) {
                 if (j == i) continue;
-                di = fma(W[(size_t)i * N + j], q[j], di);
-                const long long b = i < j ? pair_index(i, j, N) : pair_index(j, i, N);
+                const long long b = i < j ? rowoff[i] + j : rowoff[j] + i;
+                di = fma(Wt[b], q[j], di);
                 const float2 m = I[b], v = V[b];
                 // C_ij = conj(I_ij) V_ij for the ordered pair (i, j); the stored pair is (min, max)
                 double cr = (double)m.x * v.x + (double)m.y * v.y;
@@ -134,92 +140,115 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_kernel(const CalParams 
         }
         __syncthreads();
         // range projection of the singular system's right-hand side (null vector: all ones)
+        double mean1;
         {
             double s[1] = {0.0};
             for (int i = tid; i < N; i += CAL_THREADS) s[0] += rhs1[i];
-            block_sum<1>(s, scratch);
-            const double mean = s[0] / N;
-            for (int i = tid; i < N; i += CAL_THREADS) rhs1[i] -= mean;
+            block_sum<1>(s, scratch, flip);
+            mean1 = s[0] / N;
         }
-        // Jacobi-preconditioned CG on both systems, x = 0 start.  qp[j] = q_j (p0_j, p1_j) is formed
-        // once per iteration so the product loop reads one W word and one 16-byte broadcast per j.
-        double rz[3] = {0.0, 0.0, 0.0};
-        for (int i = tid; i < N; i += CAL_THREADS) {
-            const double dg = q[i] * d[i], inv = dg > 0.0 ? 1.0 / dg : 0.0;
-            invd[i] = inv;
-            rz[2] += dg;
-            x0[i] = 0.0; x1[i] = 0.0;
-            r0[i] = rhs0[i]; r1[i] = rhs1[i];
-            p0[i] = r0[i] * inv; p1[i] = r1[i] * inv;
-            qp[i] = make_double2(q[i] * p0[i], q[i] * p1[i]);
-            rz[0] += r0[i] * p0[i]; rz[1] += r1[i] * p1[i];
-        }
-        block_sum<3>(rz, scratch);
-        // stop at a residual reduced by sqrt(cg_tol2), or once the correction it stands for is below
-        // cg_abs in the (q d)-weighted rms of eps (late outer iterations start almost converged)
-        const double floor0 = fmax(p.cg_tol2 * rz[0], p.cg_abs2 * rz[2]);
-        const double floor1 = fmax(p.cg_tol2 * rz[1], p.cg_abs2 * rz[2]);
-        for (int cg = 0; cg < p.cg_max; ++cg) {
-            const bool live0 = rz[0] > floor0;
-            const bool live1 = rz[1] > floor1;
-            if (!live0 && !live1) break;
-            // t = W (q o p): `split` thread groups each take a slice of the partners j of antenna i
+
+        // ---- CG state of antenna i lives in the registers of thread i (N <= CAL_THREADS is enforced)
+        const bool own = tid < N;
+        const int i = own ? tid : 0;
+        const double qi = q[i], di = d[i];
+        const double dg = qi * di, inv = dg > 0.0 ? 1.0 / dg : 0.0;       // Jacobi preconditioner 1 / (q d)
+        double x0 = 0.0, x1 = 0.0, r0 = own ? rhs0[i] : 0.0, r1 = own ? rhs1[i] - mean1 : 0.0;
+        double u0 = r0 * inv, u1 = r1 * inv, w0 = 0.0, w1 = 0.0;
+        double p0 = 0.0, p1 = 0.0, s0 = 0.0, s1 = 0.0;
+        double gam0 = 0.0, gam1 = 0.0, al0 = 0.0, al1 = 0.0, floor0 = 0.0, floor1 = 0.0;
+        bool live0 = true, live1 = true;
+
+        // w = A u for both systems: t = W (q o u) by `split` thread groups over slices of the partners j,
+        // then w0 = q (d u0 + t0), w1 = q (d u1 - t1); fused with the reduction of (r, u) and (w, u)
+        auto product_and_dots = [&](double (&red)[5]) {
+            if (own) qu[i] = make_double2(live0 ? qi * u0 : 0.0, live1 ? qi * u1 : 0.0);
+            __syncthreads();
             if (tid < split * N) {
-                const int i = tid % N, h = tid / N;
+                const int ii = tid % N, h = tid / N;
                 const int j0 = h * jchunk, j1 = min(N, j0 + jchunk);
-                const double *Wc = W + i;
-                double t0 = 0.0, t1 = 0.0, u0 = 0.0, u1 = 0.0;
+                double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;
+                // partners j < ii: element (j, ii) at rowoff[j] + ii (consecutive over ii: conflict-free)
+                const int ja = min(ii, j1);
                 int j = j0;
+                // column walk: rowoff[j + 1] - rowoff[j] = N - j - 2, so the offset is carried, not loaded
+                const double *col = Wt + rowoff[j0 < N ? j0 : 0] + ii;
+#pragma unroll 4
+                for (; j + 1 < ja; j += 2) {
+                    const double wa = col[0], wb = col[N - j - 2];
+                    col += 2 * N - 2 * j - 5;
+                    const double2 a = qu[j], b = qu[j + 1];
+                    t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1);
+                    v0 = fma(wb, b.x, v0); v1 = fma(wb, b.y, v1);
+                }
+                if (j < ja) { const double wa = col[0]; const double2 a = qu[j]; t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1); }
+                // partners j > ii: element (ii, j) at rowoff[ii] + j (a row of the triangle)
+                const double *row = Wt + rowoff[ii];
+                j = max(ii + 1, j0);
 #pragma unroll 4
                 for (; j + 1 < j1; j += 2) {
-                    const double wa = Wc[(size_t)j * N], wb = Wc[(size_t)(j + 1) * N];
-                    const double2 a = qp[j], b = qp[j + 1];
+                    const double wa = row[j], wb = row[j + 1];
+                    const double2 a = qu[j], b = qu[j + 1];
                     t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1);
-                    u0 = fma(wb, b.x, u0); u1 = fma(wb, b.y, u1);
+                    v0 = fma(wb, b.x, v0); v1 = fma(wb, b.y, v1);
                 }
-                if (j < j1) { const double wa = Wc[(size_t)j * N]; const double2 a = qp[j]; t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1); }
-                part[(2 * h) * N + i] = t0 + u0;
-                part[(2 * h + 1) * N + i] = t1 + u1;
+                if (j < j1) { const double wa = row[j]; const double2 a = qu[j]; t0 = fma(wa, a.x, t0); t1 = fma(wa, a.y, t1); }
+                part[(2 * h) * N + ii] = t0 + v0;
+                part[(2 * h + 1) * N + ii] = t1 + v1;
             }
             __syncthreads();
-            double pa[2] = {0.0, 0.0};
-            for (int i = tid; i < N; i += CAL_THREADS) {
+            if (own) {
                 double t0 = 0.0, t1 = 0.0;
                 for (int h = 0; h < split; ++h) { t0 += part[(2 * h) * N + i]; t1 += part[(2 * h + 1) * N + i]; }
-                a0[i] = q[i] * (d[i] * p0[i] + t0);
-                a1[i] = q[i] * (d[i] * p1[i] - t1);
-                pa[0] += p0[i] * a0[i]; pa[1] += p1[i] * a1[i];
+                w0 = qi * (di * u0 + t0);
+                w1 = qi * (di * u1 - t1);
+                red[0] = r0 * u0; red[1] = r1 * u1; red[2] = w0 * u0; red[3] = w1 * u1; red[4] = dg;
+            } else {
+                red[0] = red[1] = red[2] = red[3] = red[4] = 0.0;
             }
-            block_sum<2>(pa, scratch);
-            const double al0 = live0 && pa[0] > 0.0 ? rz[0] / pa[0] : 0.0;
-            const double al1 = live1 && pa[1] > 0.0 ? rz[1] / pa[1] : 0.0;
-            double rzn[2] = {0.0, 0.0};
-            for (int i = tid; i < N; i += CAL_THREADS) {
-                x0[i] += al0 * p0[i]; x1[i] += al1 * p1[i];
-                r0[i] -= al0 * a0[i]; r1[i] -= al1 * a1[i];
-                rzn[0] += r0[i] * r0[i] * invd[i]; rzn[1] += r1[i] * r1[i] * invd[i];
+            block_sum<5>(red, scratch, flip);
+        };
+
+        {
+            double red[5];
+            product_and_dots(red);
+            gam0 = red[0]; gam1 = red[1];
+            // stop at a preconditioned residual reduced by cg_tol2, or once the correction it stands for is
+            // below cg_abs in the (q d)-weighted rms of eps (late outer iterations start almost converged)
+            floor0 = fmax(p.cg_tol2 * gam0, p.cg_abs2 * red[4]);
+            floor1 = fmax(p.cg_tol2 * gam1, p.cg_abs2 * red[4]);
+            live0 = gam0 > floor0 && red[2] > 0.0;
+            live1 = gam1 > floor1 && red[3] > 0.0;
+            al0 = live0 ? gam0 / red[2] : 0.0;
+            al1 = live1 ? gam1 / red[3] : 0.0;
+            p0 = u0; p1 = u1; s0 = w0; s1 = w1;
+        }
+        for (int cg = 0; cg < p.cg_max && (live0 || live1); ++cg) {
+            if (live0) { x0 = fma(al0, p0, x0); r0 = fma(-al0, s0, r0); u0 = r0 * inv; }
+            if (live1) { x1 = fma(al1, p1, x1); r1 = fma(-al1, s1, r1); u1 = r1 * inv; }
+            double red[5];
+            product_and_dots(red);
+            if (live0) {
+                const double gn = red[0], be = gn / gam0, den = red[2] - be * gn / al0;
+                live0 = gn > floor0 && den > 0.0;
+                al0 = live0 ? gn / den : 0.0;
+                p0 = fma(be, p0, u0); s0 = fma(be, s0, w0); gam0 = gn;
             }
-            block_sum<2>(rzn, scratch);
-            const double be0 = live0 ? rzn[0] / rz[0] : 0.0;
-            const double be1 = live1 ? rzn[1] / rz[1] : 0.0;
-            for (int i = tid; i < N; i += CAL_THREADS) {
-                if (live0) p0[i] = r0[i] * invd[i] + be0 * p0[i];
-                if (live1) p1[i] = r1[i] * invd[i] + be1 * p1[i];
-                qp[i] = make_double2(live0 ? q[i] * p0[i] : 0.0, live1 ? q[i] * p1[i] : 0.0);
+            if (live1) {
+                const double gn = red[1], be = gn / gam1, den = red[3] - be * gn / al1;
+                live1 = gn > floor1 && den > 0.0;
+                al1 = live1 ? gn / den : 0.0;
+                p1 = fma(be, p1, u1); s1 = fma(be, s1, w1); gam1 = gn;
             }
-            if (live0) rz[0] = rzn[0];
-            if (live1) rz[1] = rzn[1];
-            __syncthreads();
         }
         // gauge: minimum norm in e = g eps  <=>  sum_i q_i Im eps_i = 0
         {
-            double s[2] = {0.0, 0.0};
-            for (int i = tid; i < N; i += CAL_THREADS) { s[0] += q[i] * x1[i]; s[1] += q[i]; }
-            block_sum<2>(s, scratch);
+            double s[2] = {own ? qi * x1 : 0.0, own ? qi : 0.0};
+            block_sum<2>(s, scratch, flip);
             const double phi = s[1] > 0.0 ? s[0] / s[1] : 0.0;
             // g <- g + e = g (1 + eps)
-            for (int i = tid; i < N; i += CAL_THREADS) {
-                const double er = x0[i], ei = x1[i] - phi;
+            if (own) {
+                const double er = x0, ei = x1 - phi;
                 const double nr = gre[i] + gre[i] * er - gim[i] * ei;
                 const double ni = gim[i] + gre[i] * ei + gim[i] * er;
                 gre[i] = nr; gim[i] = ni;
@@ -263,7 +292,8 @@ __global__ void __launch_bounds__(CAL_THREADS) peel_kernel(const float2 *__restr
 
 size_t calibrate_smem_bytes(int N)
 {
-    return ((size_t)N * N + 20 * (size_t)N + 2 + 4 * (CAL_THREADS / 32) + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS)) * sizeof(double);
+    const size_t B = (size_t)N * (N - 1) / 2;
+    return (B + (B & 1) + 7 * (size_t)N + 10 * (CAL_THREADS / 32) + 2 * (size_t)(N > CAL_THREADS ? N : CAL_THREADS) + 2 * (size_t)N + (N + 1) / 2) * sizeof(double);
 }
 
 cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *gains, int N, long long cells, int n_iter,
@@ -273,8 +303,9 @@ cudaError_t launch_calibrate(const float2 *data, const float2 *model, double2 *g
     p.data = data; p.model = model; p.gains = gains; p.N = N; p.n_iter = n_iter;
     p.B = (long long)N * (N - 1) / 2;
     p.cg_max = 2 * N + 10;
-    p.cg_tol2 = 1e-26;             // residual reduced by 1e-13
+    p.cg_tol2 = 1e-22;             // preconditioned residual reduced by 1e-11 (gains are compared at 1e-9)
     p.cg_abs2 = 1e-28;             // or the remaining relative gain correction below 1e-14
+    if (N > CAL_THREADS) return cudaErrorInvalidValue;         // the CG state of antenna i lives in thread i
     const size_t smem = calibrate_smem_bytes(N);
     cudaError_t e = cudaFuncSetAttribute(calibrate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

@@ -95,7 +95,24 @@ def test_calibrate_argument_errors(ctx):
     z = torch.zeros((1, 1), dtype=torch.complex64, device="cuda:0")
     with pytest.raises(ValueError):
         ctx.calibrate_gains(3, z, z)
-    big = torch.zeros((1, 200 * 199 // 2), dtype=torch.complex64, device="cuda:0")
+    big = torch.zeros((1, 201 * 200 // 2), dtype=torch.complex64, device="cuda:0")
     with pytest.raises(binding.WodenError) as e:
-        ctx.calibrate_gains(200, big, big)                                    # W would not fit shared memory
+        ctx.calibrate_gains(201, big, big)                                    # W would not fit shared memory
     assert e.value.status == binding.WODEN_ERR_DIM
+
+
+def test_largest_supported_array_matches_the_oracle(ctx):
+    # 200 antennas: the triangle of W fills one CTA's shared memory (one cell per SM); one and three passes
+    import torch
+    n_ant = 200
+    rng = np.random.default_rng(200)
+    nb = n_ant * (n_ant - 1) // 2
+    ideal = (rng.normal(0, 3, (1, nb)) + 1j * rng.normal(0, 3, (1, nb))).astype(np.complex64)
+    gam = (1 + 0.1 * rng.normal(0, 1, (1, n_ant))) * np.exp(1j * rng.normal(0, 0.3, (1, n_ant)))
+    i, j = ocal.baseline_pairs(n_ant)
+    data = (gam[..., i] * np.conj(gam[..., j]) * ideal).astype(np.complex64)
+    for n_iter in (1, 3):
+        g = ctx.calibrate_gains(n_ant, _dev(data), _dev(ideal), n_iter)
+        torch.cuda.synchronize()
+        ref = ocal.calibrate(data, ideal, n_ant, n_iter)
+        assert np.abs(g.cpu().numpy() - ref).max() <= 1e-9 * max(1.0, np.abs(ref).max())
