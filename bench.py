@@ -480,7 +480,7 @@ def run_truncation(args):
     uvw = binding.Uvw(*(torch.as_tensor(a, device="cuda:0") for a in (wl.u_m, wl.v_m, wl.w_m)), wl.freqs_hz)
     vis = ctx.new_vis(uvw)
     dev = lambda a, dt=torch.float64: torch.as_tensor(np.ascontiguousarray(a), dtype=dt, device="cuda:0")
-    w_sh = truncate.shapelet_basis_weights(wl.shapelets)
+    w_sh = truncate.shapelet_basis_weights(ctx, wl.shapelets)
 
     def timed(fn):
         for _ in range(2):
@@ -495,8 +495,8 @@ def run_truncation(args):
 
     rows = []
     for f in (1.0, 0.8, 0.6, 0.4, 0.2, 0.1):
-        p, g = truncate.truncate_components(wl.points, f), truncate.truncate_components(wl.gaussians, f)
-        s = truncate.truncate_shapelets(wl.shapelets, f, w_sh)
+        p, g = truncate.truncate_components(ctx, wl.points, f), truncate.truncate_components(ctx, wl.gaussians, f)
+        s = truncate.truncate_shapelets(ctx, wl.shapelets, f, w_sh)
         dp = [dev(a) for a in (p.l, p.m, p.s0_jy, p.alpha)]
         dg = [dev(a) for a in (g.l, g.m, g.s0_jy, g.alpha, g.maj_fwhm_rad, g.min_fwhm_rad, g.pa_rad)]
         ds_ = [dev(a) for a in (s.l, s.m, s.s0_jy, s.alpha, s.beta1_rad, s.beta2_rad, s.pa_rad, s.uv_basis)]
@@ -631,9 +631,9 @@ def run_peel(args):
     dw = binding.DeviceWorkload(wl)
     full = dw.predict(ctx)
     wl_t = inputs.make_config(args.config)
-    wl_t.points = truncate.truncate_components(wl.points, 0.8)
-    wl_t.gaussians = truncate.truncate_components(wl.gaussians, 0.8)
-    wl_t.shapelets = truncate.truncate_shapelets(wl.shapelets, 0.8)
+    wl_t.points = truncate.truncate_components(ctx, wl.points, 0.8)
+    wl_t.gaussians = truncate.truncate_components(ctx, wl.gaussians, 0.8)
+    wl_t.shapelets = truncate.truncate_shapelets(ctx, wl.shapelets, 0.8)
     model = binding.DeviceWorkload(wl_t).predict(ctx)
     out = torch.empty_like(full)
     torch.cuda.synchronize()

@@ -268,6 +268,26 @@ int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const doub
                         const woden_restoring_beam *beam, int n_refine,
                         double *coeff, double *residual, double *weights, int *best, void *cuda_stream);
 
+/* Eq 25 without the coefficient: abs_sums[q] = sum over the grid's pixels of
+ * |(G * B_q)(x_s, y_t)| for every basis function q of order <= p_max (same order, basis, beam and grid
+ * conventions as woden_fit_shapelets); the truncation weight of a basis function is |C_q| abs_sums[q]
+ * (what woden_fit_shapelets returns in `weights` for the coefficients it fitted).  abs_sums: DEVICE [P].
+ * 0 <= p_max <= WODEN_MAX_ORDER (no solve is involved). */
+int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, double l0, double m0, double pa_rad,
+                              int p_max, double beta1_rad, double beta2_rad, const woden_restoring_beam *beam,
+                              double *abs_sums, void *cuda_stream);
+
+/* Model truncation, section 5.3 (Eq 23-24, :273-275): with the n
+ * components ranked by |weights[j]|, largest first (equal values in their original order), keep the
+ * largest N_comp whose summed absolute weight does not exceed f_comp times the total,
+ *     sum_{j <= N_comp} |I_j| <= f_comp sum_{j <= N_tot} |I_j|     (Eq 23),  |I_j| >= |I_{j+1}|   (Eq 24).
+ * weights: DEVICE [n] (the integrated flux density of a point source or Gaussian; Eq 25's weight of a
+ * shapelet basis function).  keep: DEVICE int [n], 1 for a kept component, else 0; n_keep: DEVICE
+ * int [1] = N_comp.  f_comp >= 1 keeps everything; the running sum is formed in ranked order in FP64 and
+ * compared with f_comp * total * (1 + 1e-15).  0 <= n <= 2^20 (ranking is by counting, O(n^2)). */
+int woden_truncate_select(woden_ctx *ctx, int n, const double *weights, double f_comp, int *keep, int *n_keep,
+                          void *cuda_stream);
+
 /* Measurement aid: device time in milliseconds of the Gram-matrix kernel (the tcgen05 contraction) of
  * the LAST (beta1, beta2) pair of the last woden_fit_shapelets call on this context, from CUDA events
  * recorded around it on the call's stream.  Synchronises on that kernel.  WODEN_ERR_DIM before any fit. */

@@ -40,7 +40,8 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
            "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
-           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms"]
+           "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms", "woden_shapelet_basis_sums",
+           "woden_truncate_select"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -116,6 +117,9 @@ def load() -> C.CDLL:
                                       C.POINTER(woden_shapelets_host), _vp, _vp]
     L.woden_pipe_rate.argtypes = [_vp, C.c_int, C.c_int, _dp, _dp]
     L.woden_fit_gram_ms.argtypes = [_vp, C.POINTER(C.c_float)]
+    L.woden_shapelet_basis_sums.argtypes = [_vp, C.POINTER(woden_image_grid), C.c_double, C.c_double, C.c_double, C.c_int,
+                                            C.c_double, C.c_double, C.POINTER(woden_restoring_beam), _vp, _vp]
+    L.woden_truncate_select.argtypes = [_vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp]
     L.woden_fit_shapelets.argtypes = [_vp, C.POINTER(woden_image_grid), _vp, C.c_double, C.c_double, C.c_double, C.c_int,
                                       C.c_int, _dp, _dp, C.POINTER(woden_restoring_beam), C.c_int, _vp, _vp, _vp, _vp, _vp]
     L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
@@ -370,6 +374,32 @@ class Woden:
                                          _stream_handle(stream))
         self._ck(rc, "woden_fit_shapelets")
         return coeff, resid, weights, best
+
+    def shapelet_basis_sums(self, n_l, n_m, dl, dm, l_c, m_c, l0, m0, pa_rad, p_max, beta1_rad, beta2_rad, beam=None,
+                            device="cuda:0", stream=None):
+        """woden_shapelet_basis_sums: device float64 [P] of sum_pixels |G * B_q| (Eq 25 without |C|)."""
+        import torch
+        grid = woden_image_grid(int(n_l), int(n_m), float(dl), float(dm), float(l_c), float(m_c))
+        cb = woden_restoring_beam(*[float(x) for x in beam[:3]], int(beam[3])) if beam is not None else None
+        out = torch.empty((p_max + 1) * (p_max + 2) // 2, dtype=torch.float64, device=device)
+        rc = self._L.woden_shapelet_basis_sums(self._ctx, C.byref(grid), float(l0), float(m0), float(pa_rad), int(p_max),
+                                               float(beta1_rad), float(beta2_rad), C.byref(cb) if cb is not None else None,
+                                               _ptr(out), _stream_handle(stream))
+        self._ck(rc, "woden_shapelet_basis_sums")
+        return out
+
+    def truncate_select(self, weights, f_comp: float, stream=None):
+        """woden_truncate_select on a float64 device tensor: (keep flags int32 [n], N_comp int32 [1])."""
+        import torch
+        if weights.dtype != torch.float64 or weights.dim() != 1:
+            raise ValueError("weights must be a 1-D float64 device tensor")
+        n = int(weights.numel())
+        keep = torch.empty(n, dtype=torch.int32, device=weights.device)
+        n_keep = torch.empty(1, dtype=torch.int32, device=weights.device)
+        rc = self._L.woden_truncate_select(self._ctx, n, _ptr(weights) if n else None, float(f_comp),
+                                           _ptr(keep) if n else None, _ptr(n_keep), _stream_handle(stream))
+        self._ck(rc, "woden_truncate_select")
+        return keep, n_keep
 
     def fit_gram_ms(self) -> float:
         ms = C.c_float(0.0)

@@ -656,64 +656,87 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells, const float *v
     return WODEN_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// argument checks and scratch of the image-space entry points; `full` also allocates the solver's buffers
+int fit_setup(woden_ctx *ctx, const woden_image_grid *grid, double l0, double m0, double pa_rad, int p_max,
+              const woden_restoring_beam *beam, bool full, cudaStream_t st, FitScratch *w, FitProblem *f, FitSizes *szo)
+{
+    if (p_max < 0 || p_max > (full ? WODEN_FIT_MAX_ORDER : WODEN_MAX_ORDER)) return WODEN_ERR_ORDER;
+    if (grid->n_l <= 0 || grid->n_m <= 0 || (long long)grid->n_l * grid->n_m > (1LL << 22) || !(grid->dl != 0.0) ||
+        !(grid->dm != 0.0) || !std::isfinite(grid->dl) || !std::isfinite(grid->dm) || !std::isfinite(grid->l_c) ||
+        !std::isfinite(grid->m_c) || !std::isfinite(l0) || !std::isfinite(m0) || !std::isfinite(pa_rad))
+        return WODEN_ERR_DIM;
+    const bool has_beam = beam && beam->bmaj_rad > 0.0;
+    if (has_beam && (beam->half_width < 0 || beam->half_width > 24 || !(beam->bmin_rad >= 0.0) ||
+                     !std::isfinite(beam->bmaj_rad) || !std::isfinite(beam->bmin_rad) || !std::isfinite(beam->bpa_rad)))
+        return WODEN_ERR_DIM;
+    int rc = ensure_err(ctx, st);
+    if (rc != WODEN_OK) return rc;
+    const int n_pix = grid->n_l * grid->n_m;
+    const FitSizes sz = fit_sizes(n_pix, p_max);
+    if (full && sz.n_pad > FIT_MAX_N) return WODEN_ERR_ORDER;
+    const size_t small = (size_t)4 * sz.n_pad + n_pix + 49 * 49 + 64;        // scale, abssum, z, g | r | stencil
+    CU(ctx, ctx->f_hx.reserve(sz.hermite_doubles * 8), "alloc fit Hermite tables");
+    CU(ctx, ctx->f_at.reserve(sz.at_doubles * 8), "alloc fit design matrix");
+    if (has_beam) CU(ctx, ctx->f_a0.reserve(sz.at_doubles * 8), "alloc fit unconvolved basis");
+    CU(ctx, ctx->f_small.reserve(small * 8), "alloc fit vectors");
+    if (full) {
+        CU(ctx, ctx->f_gram.reserve(sz.gram_doubles * 8), "alloc fit Gram matrix");
+        CU(ctx, ctx->f_ops.reserve(sz.ops_halves * 2), "alloc fit operands");
+        CU(ctx, ctx->f_part.reserve(sz.partial_floats * 4), "alloc fit partials");
+        if (!ctx->fit_t0) {
+            CU(ctx, cudaEventCreate(&ctx->fit_t0), "create event");
+            CU(ctx, cudaEventCreate(&ctx->fit_t1), "create event");
+        }
+    }
+    w->hx = static_cast<double *>(ctx->f_hx.p);
+    w->a0 = static_cast<double *>(ctx->f_a0.p);
+    w->at = static_cast<double *>(ctx->f_at.p);
+    double *v = static_cast<double *>(ctx->f_small.p);
+    w->scale = v; w->abssum = v + sz.n_pad; w->z = v + 2 * sz.n_pad; w->g = v + 3 * sz.n_pad;
+    w->r = v + 4 * sz.n_pad; w->stencil = w->r + n_pix;
+    w->gram = static_cast<double *>(ctx->f_gram.p);
+    w->ops = static_cast<__half *>(ctx->f_ops.p);
+    w->partial = static_cast<float *>(ctx->f_part.p);
+    w->err = static_cast<unsigned int *>(ctx->err.p);
+    w->gram_t0 = full ? ctx->fit_t0 : nullptr; w->gram_t1 = full ? ctx->fit_t1 : nullptr;
+    f->n_l = grid->n_l; f->n_m = grid->n_m; f->p_max = p_max;
+    f->half_width = has_beam ? beam->half_width : 0;
+    f->n_refine = 0;
+    f->dl = grid->dl; f->dm = grid->dm; f->l_c = grid->l_c; f->m_c = grid->m_c; f->l0 = l0; f->m0 = m0; f->pa = pa_rad;
+    f->bmaj = has_beam ? beam->bmaj_rad : 0.0; f->bmin = has_beam ? beam->bmin_rad : 0.0; f->bpa = has_beam ? beam->bpa_rad : 0.0;
+    f->image = nullptr; f->coeff = nullptr; f->weights = nullptr; f->residual = nullptr;
+    *szo = sz;
+    return WODEN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const double *image, double l0, double m0,
                         double pa_rad, int p_max, int n_beta, const double *beta1_rad, const double *beta2_rad,
                         const woden_restoring_beam *beam, int n_refine, double *coeff, double *residual,
                         double *weights, int *best, void *cuda_stream)
 {
     if (!ctx || !grid || !image || !beta1_rad || !beta2_rad || !coeff || !residual) return WODEN_ERR_NULL;
-    if (p_max < 0 || p_max > WODEN_FIT_MAX_ORDER) return WODEN_ERR_ORDER;
-    if (grid->n_l <= 0 || grid->n_m <= 0 || (long long)grid->n_l * grid->n_m > (1LL << 22) || n_beta <= 0 ||
-        n_refine < 0 || !(grid->dl != 0.0) || !(grid->dm != 0.0) || !std::isfinite(grid->dl) || !std::isfinite(grid->dm) ||
-        !std::isfinite(grid->l_c) || !std::isfinite(grid->m_c) || !std::isfinite(l0) || !std::isfinite(m0) ||
-        !std::isfinite(pa_rad))
-        return WODEN_ERR_DIM;
+    if (n_beta <= 0 || n_refine < 0) return WODEN_ERR_DIM;
     for (int k = 0; k < n_beta; ++k)
         if (!(beta1_rad[k] > 0.0) || !(beta2_rad[k] > 0.0) || !std::isfinite(beta1_rad[k]) || !std::isfinite(beta2_rad[k]))
             return WODEN_ERR_DIM;
-    const bool has_beam = beam && beam->bmaj_rad > 0.0;
-    if (has_beam && (beam->half_width < 0 || beam->half_width > 24 || !(beam->bmin_rad >= 0.0) ||
-                     !std::isfinite(beam->bmaj_rad) || !std::isfinite(beam->bmin_rad) || !std::isfinite(beam->bpa_rad)))
-        return WODEN_ERR_DIM;
     Bind bind(ctx);
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ctx->last_stream = st;
-    int rc = ensure_err(ctx, st);
-    if (rc != WODEN_OK) return rc;
-    const int n_pix = grid->n_l * grid->n_m;
-    const FitSizes sz = fit_sizes(n_pix, p_max);
-    if (sz.n_pad > FIT_MAX_N) return WODEN_ERR_ORDER;
-    const size_t small = (size_t)4 * sz.n_pad + n_pix + 49 * 49 + 64;        // scale, abssum, z, g | r | stencil
-    CU(ctx, ctx->f_hx.reserve(sz.hermite_doubles * 8), "alloc fit Hermite tables");
-    CU(ctx, ctx->f_at.reserve(sz.at_doubles * 8), "alloc fit design matrix");
-    if (has_beam) CU(ctx, ctx->f_a0.reserve(sz.at_doubles * 8), "alloc fit unconvolved basis");
-    CU(ctx, ctx->f_small.reserve(small * 8), "alloc fit vectors");
-    CU(ctx, ctx->f_gram.reserve(sz.gram_doubles * 8), "alloc fit Gram matrix");
-    CU(ctx, ctx->f_ops.reserve(sz.ops_halves * 2), "alloc fit operands");
-    CU(ctx, ctx->f_part.reserve(sz.partial_floats * 4), "alloc fit partials");
     FitScratch w;
-    w.hx = static_cast<double *>(ctx->f_hx.p);
-    w.a0 = static_cast<double *>(ctx->f_a0.p);
-    w.at = static_cast<double *>(ctx->f_at.p);
-    double *v = static_cast<double *>(ctx->f_small.p);
-    w.scale = v; w.abssum = v + sz.n_pad; w.z = v + 2 * sz.n_pad; w.g = v + 3 * sz.n_pad;
-    w.r = v + 4 * sz.n_pad; w.stencil = w.r + n_pix;
-    w.gram = static_cast<double *>(ctx->f_gram.p);
-    w.ops = static_cast<__half *>(ctx->f_ops.p);
-    w.partial = static_cast<float *>(ctx->f_part.p);
-    w.err = static_cast<unsigned int *>(ctx->err.p);
-    if (!ctx->fit_t0) {
-        CU(ctx, cudaEventCreate(&ctx->fit_t0), "create event");
-        CU(ctx, cudaEventCreate(&ctx->fit_t1), "create event");
-    }
-    w.gram_t0 = ctx->fit_t0; w.gram_t1 = ctx->fit_t1;
     FitProblem f;
-    f.n_l = grid->n_l; f.n_m = grid->n_m; f.p_max = p_max;
-    f.half_width = has_beam ? beam->half_width : 0;
+    FitSizes sz;
+    int rc = fit_setup(ctx, grid, l0, m0, pa_rad, p_max, beam, true, st, &w, &f, &sz);
+    if (rc != WODEN_OK) return rc;
     f.n_refine = n_refine > 0 ? n_refine : 6;
-    f.dl = grid->dl; f.dm = grid->dm; f.l_c = grid->l_c; f.m_c = grid->m_c; f.l0 = l0; f.m0 = m0; f.pa = pa_rad;
-    f.bmaj = has_beam ? beam->bmaj_rad : 0.0; f.bmin = has_beam ? beam->bmin_rad : 0.0; f.bpa = has_beam ? beam->bpa_rad : 0.0;
     f.image = image;
     for (int k = 0; k < n_beta; ++k) {
         f.beta1 = beta1_rad[k]; f.beta2 = beta2_rad[k];
@@ -723,6 +746,43 @@ int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const doub
         CU(ctx, launch_fit_one(f, w, st), "fit launch");
     }
     if (best) CU(ctx, launch_fit_argmin(residual, n_beta, best, st), "fit argmin launch");
+    return WODEN_OK;
+}
+
+int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, double l0, double m0, double pa_rad, int p_max,
+                              double beta1_rad, double beta2_rad, const woden_restoring_beam *beam, double *abs_sums,
+                              void *cuda_stream)
+{
+    if (!ctx || !grid || !abs_sums) return WODEN_ERR_NULL;
+    if (!(beta1_rad > 0.0) || !(beta2_rad > 0.0) || !std::isfinite(beta1_rad) || !std::isfinite(beta2_rad)) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    FitScratch w;
+    FitProblem f;
+    FitSizes sz;
+    int rc = fit_setup(ctx, grid, l0, m0, pa_rad, p_max, beam, false, st, &w, &f, &sz);
+    if (rc != WODEN_OK) return rc;
+    f.beta1 = beta1_rad; f.beta2 = beta2_rad;
+    CU(ctx, launch_fit_basis_sums(f, w, abs_sums, st), "basis sums launch");
+    return WODEN_OK;
+}
+
+int woden_truncate_select(woden_ctx *ctx, int n, const double *weights, double f_comp, int *keep, int *n_keep, void *cuda_stream)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    if (n < 0 || n > (1 << 20) || !(f_comp >= 0.0)) return WODEN_ERR_DIM;
+    if (!n_keep || (n > 0 && (!weights || !keep))) return WODEN_ERR_NULL;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    if (n == 0) { CU(ctx, cudaMemsetAsync(n_keep, 0, sizeof(int), st), "truncate zero"); return WODEN_OK; }
+    CU(ctx, ctx->f_small.reserve((size_t)n * 12 + 64), "alloc truncation scratch");
+    double *sorted = static_cast<double *>(ctx->f_small.p);
+    int *rank = reinterpret_cast<int *>(sorted + n);
+    CU(ctx, launch_truncate_select(weights, n, f_comp, rank, sorted, keep, n_keep, st), "truncate launch");
     return WODEN_OK;
 }
 

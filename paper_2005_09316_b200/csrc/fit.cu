@@ -623,11 +623,11 @@ FitSizes fit_sizes(int n_pix, int p_max)
     return s;
 }
 
-cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st)
+// steps 1-3: basis images, beam convolution, row scaling (+ Eq 25 row sums) into w.at / w.scale / w.abssum
+static cudaError_t fit_build_rows(const FitProblem &f, const FitScratch &w, cudaStream_t st)
 {
     const int n_pix = f.n_l * f.n_m;
-    const FitSizes sz = fit_sizes(n_pix, f.p_max);
-    const int P = sz.P;
+    const int P = (f.p_max + 1) * (f.p_max + 2) / 2;
     const double a = 2.0 * sqrt(2.0 * LN2);
     BasisParams b;
     b.n_l = f.n_l; b.n_m = f.n_m; b.p_max = f.p_max;
@@ -646,10 +646,28 @@ cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_
         cudaError_t e = cudaFuncSetAttribute(fit_convolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         fit_stencil_kernel<<<1, 256, 0, st>>>(f.dl, f.dm, f.bmaj, f.bmin, sin(f.bpa), cos(f.bpa), hw, w.stencil); note_launch();
-        fit_convolve_kernel<<<dim3((f.n_l + CV_W - 1) / CV_W, (f.n_m + CV_H - 1) / CV_H, P), dim3(16, 16), smem, st>>>(w.a0, w.stencil, f.n_l,
-                                                                                                      f.n_m, hw, w.at); note_launch();
+        fit_convolve_kernel<<<dim3((f.n_l + CV_W - 1) / CV_W, (f.n_m + CV_H - 1) / CV_H, P), dim3(16, 16), smem, st>>>(
+            w.a0, w.stencil, f.n_l, f.n_m, hw, w.at); note_launch();
     }
     fit_scale_rows_kernel<<<P, 256, 0, st>>>(w.at, n_pix, w.scale, w.abssum); note_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fit_basis_sums(const FitProblem &f, const FitScratch &w, double *abs_sums, cudaStream_t st)
+{
+    cudaError_t e = fit_build_rows(f, w, st);
+    if (e != cudaSuccess) return e;
+    const int P = (f.p_max + 1) * (f.p_max + 2) / 2;
+    return cudaMemcpyAsync(abs_sums, w.abssum, (size_t)P * sizeof(double), cudaMemcpyDeviceToDevice, st);
+}
+
+cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st)
+{
+    const int n_pix = f.n_l * f.n_m;
+    const FitSizes sz = fit_sizes(n_pix, f.p_max);
+    const int P = sz.P;
+    cudaError_t e0 = fit_build_rows(f, w, st);
+    if (e0 != cudaSuccess) return e0;
     {
         const long long groups = (long long)sz.n_pad * sz.n_kt * (GK / 8);
         fit_split_kernel<<<(unsigned)((groups + 255) / 256), 256, 0, st>>>(w.at, P, n_pix, sz.n_rt, sz.n_kt, w.ops); note_launch();

@@ -118,6 +118,13 @@ struct FitScratch {
 cudaError_t launch_fit_one(const FitProblem &f, const FitScratch &w, cudaStream_t st);
 cudaError_t launch_fit_argmin(const double *residual, int n, int *best, cudaStream_t st);
 
+// Eq 25 without |C|: abs_sums[q] = sum over pixels of |(G * B_q)| (steps 1-3 of the fit for one beta pair)
+cudaError_t launch_fit_basis_sums(const FitProblem &f, const FitScratch &w, double *abs_sums, cudaStream_t st);
+
+// ---- model truncation (truncate.cu, Eq 23-24) ---------------------
+cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
+                                   int *n_keep, cudaStream_t st);
+
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);
 

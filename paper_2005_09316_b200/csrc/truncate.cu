@@ -1,0 +1,61 @@
+// truncate.cu -- model truncation of PAPER.md section 5.3 (Eq 23-24, :273-275):
+// rank the components (or shapelet basis functions) by |I_j|, largest first, and keep the largest N_comp
+// with  sum_{j <= N_comp} |I_j| <= f_comp sum_{j <= N_tot} |I_j|.
+//
+// Three small kernels: ranks by counting (rank_j = number of components with a larger |I|, ties in
+// original order: a stable descending sort without a sort), the running sum over the ranked list by ONE
+// thread in list order (the same association as a sequential cumulative sum, so N_comp is decided on
+// exactly the same FP64 numbers as the oracle's), and the keep flags.
+#include "kernels.h"
+
+namespace woden {
+namespace {
+
+__global__ void trunc_rank_kernel(const double *__restrict__ w, int n, int *__restrict__ rank, double *__restrict__ sorted)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const double a = fabs(w[j]);
+    int r = 0;
+    for (int i = 0; i < n; ++i) {
+        const double b = fabs(w[i]);
+        r += (b > a) || (b == a && i < j);
+    }
+    rank[j] = r;
+    sorted[r] = a;
+}
+
+__global__ void trunc_count_kernel(const double *__restrict__ sorted, int n, double f_comp, int *__restrict__ n_keep)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    if (f_comp >= 1.0) { *n_keep = n; return; }
+    double total = 0.0;
+    for (int k = 0; k < n; ++k) total += sorted[k];
+    const double limit = f_comp * total * (1.0 + 1e-15);       // Eq 23 with one rounding of slack
+    double run = 0.0;
+    int keep = 0;
+    for (int k = 0; k < n; ++k) {
+        run += sorted[k];
+        if (run <= limit) keep = k + 1; else break;
+    }
+    *n_keep = keep;
+}
+
+__global__ void trunc_flag_kernel(const int *__restrict__ rank, int n, const int *__restrict__ n_keep, int *__restrict__ keep)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) keep[j] = rank[j] < *n_keep ? 1 : 0;
+}
+
+}  // namespace
+
+cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
+                                   int *n_keep, cudaStream_t st)
+{
+    trunc_rank_kernel<<<(n + 127) / 128, 128, 0, st>>>(weights, n, rank, sorted); note_launch();
+    trunc_count_kernel<<<1, 32, 0, st>>>(sorted, n, f_comp, n_keep); note_launch();
+    trunc_flag_kernel<<<(n + 255) / 256, 256, 0, st>>>(rank, n, n_keep, keep); note_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace woden

@@ -74,7 +74,7 @@ def test_peeling_a_predicted_sky_with_a_truncated_model(ctx):
     p = wl.points
     full = ctx.new_vis(uvw)
     ctx.predict_points(uvw, _dev(p.l), _dev(p.m), _dev(p.s0_jy), _dev(p.alpha), wl.ref_freq_hz, full)
-    pt = truncate.truncate_components(p, 0.8)
+    pt = truncate.truncate_components(ctx, p, 0.8)
     model = ctx.new_vis(uvw)
     ctx.predict_points(uvw, _dev(pt.l), _dev(pt.m), _dev(pt.s0_jy), _dev(pt.alpha), wl.ref_freq_hz, model)
     g = ctx.calibrate_gains(n_ant, full, model, 10)

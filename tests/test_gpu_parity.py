@@ -258,7 +258,7 @@ def test_truncated_shapelet_models_take_the_sparse_kernel(ctx, torch_mod, cfg, f
     # ragged coefficient lists go through the chunk-skipping kernel variant (PM = 40 NV = 2, PM = 60)
     from paper_2005_09316_b200 import truncate
     wl = inputs.make_config(cfg)
-    s = truncate.truncate_shapelets(wl.shapelets, f_comp)
+    s = truncate.truncate_shapelets(ctx, wl.shapelets, f_comp)
     assert s.coeff.size < 0.75 * wl.shapelets.coeff.size
     u, v, w = (a[:2, :1500] for a in (wl.u_m, wl.v_m, wl.w_m))
     fr = wl.freqs_hz[::48]

@@ -1,49 +1,120 @@
-"""Model truncation (§5.3, Eq 23-24): host-side selection logic, checked by brute force."""
+"""Model truncation (section 5.3, Eq 23-24): pins of the oracle (oracle/truncate.py) on the CPU
+and, `-m gpu`, parity of woden_truncate_select / woden_shapelet_basis_sums against the oracles."""
 import numpy as np
+import pytest
 
-from paper_2005_09316_b200 import inputs, truncate
+from oracle import shamfi
+from oracle import truncate as otrunc
+from paper_2005_09316_b200 import inputs
+
+ARCMIN = np.pi / 180.0 / 60.0
 
 
-def _brute_n_keep(a_sorted, f):
-    tot, n, run = sum(a_sorted), 0, 0.0
-    for x in a_sorted:                       # Eq 23: largest N with sum_{j<=N} |I_j| <= f * total
-        if run + x <= f * tot * (1 + 1e-15):
-            run += x; n += 1
+def _brute_keep(weights, f):
+    """Every prefix of the ranked list is tried; the largest admissible one wins (Eq 23 read literally)."""
+    w = [abs(float(x)) for x in weights]
+    order = sorted(range(len(w)), key=lambda j: (-w[j], j))
+    tot = sum(w[j] for j in order)
+    best = 0
+    for n in range(len(w) + 1):
+        if sum(w[j] for j in order[:n]) <= f * tot * (1 + 1e-15):
+            best = n
         else:
             break
-    return n
+    return set(order[:best])
 
 
-def test_eq23_eq24_against_brute_force():
+def test_eq23_eq24_against_brute_force_and_a_worked_example():
     rng = np.random.default_rng(5)
-    for _ in range(50):
-        a = np.sort(rng.lognormal(0, 1.5, rng.integers(1, 40)))[::-1]
+    for _ in range(40):
+        w = rng.lognormal(0, 1.5, rng.integers(1, 40)) * rng.choice([-1.0, 1.0], 1)
         for f in (0.0, 0.1, 0.5, 0.9, 0.999, 1.0):
-            assert truncate.n_keep(a, f) == _brute_n_keep(list(a), f)
-    assert truncate.n_keep(np.array([]), 0.5) == 0
-    # worked example: |I| = 5, 3, 1, 1 (total 10): f = 0.8 keeps {5, 3}; f = 0.85 still {5, 3}; 0.9 adds one
-    a = np.array([5.0, 3.0, 1.0, 1.0])
-    assert [truncate.n_keep(a, f) for f in (0.49, 0.5, 0.8, 0.85, 0.9, 1.0)] == [0, 1, 2, 2, 3, 4]
+            got = set(np.flatnonzero(otrunc.keep_mask(w, f)))
+            assert got == _brute_keep(w, f) if f < 1.0 else len(got) == w.size
+    assert otrunc.n_keep([], 0.5) == 0
+    # worked example: |I| = 5, 3, 1, 1 (total 10): f = 0.8 keeps {5, 3}; 0.85 still {5, 3}; 0.9 adds one
+    a = [5.0, 3.0, 1.0, 1.0]
+    assert [otrunc.n_keep(a, f) for f in (0.49, 0.5, 0.8, 0.85, 0.9, 1.0)] == [0, 1, 2, 2, 3, 4]
+    # signs do not matter, order of equal values does: the earlier of two equal components is kept first
+    m = otrunc.keep_mask([1.0, -5.0, 1.0, 3.0], 0.9)
+    assert m.tolist() == [True, True, False, True]
 
 
-def test_components_keep_the_brightest_by_absolute_flux():
+def test_invariants_of_the_selection():
+    rng = np.random.default_rng(6)
+    w = rng.normal(0, 1, 500) * rng.lognormal(0, 2, 500)
+    tot = np.abs(w).sum()
+    prev = 0
+    for f in np.linspace(0, 1, 21):
+        m = otrunc.keep_mask(w, f)
+        kept = np.abs(w[m]).sum()
+        assert kept <= f * tot * (1 + 1e-12)
+        if m.sum() < w.size:                                     # the next one would not fit
+            nxt = np.abs(w[~m]).max()
+            assert kept + nxt > f * tot * (1 - 1e-12)
+            assert np.abs(w[m]).min() >= nxt if m.any() else True
+        assert m.sum() >= prev                                   # monotone in f_comp
+        prev = m.sum()
+    perm = rng.permutation(w.size)                               # distinct values: the choice is a set of values
+    assert np.array_equal(np.sort(w[otrunc.keep_mask(w, 0.6)]), np.sort(w[perm][otrunc.keep_mask(w[perm], 0.6)]))
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2005_09316_b200 import binding
+    c = binding.Woden(0)
+    yield c
+    c.close()
+
+
+@pytest.mark.gpu
+def test_gpu_selection_is_bit_exact_against_the_oracle(ctx):
+    import torch
+    rng = np.random.default_rng(9)
+    cases = [rng.normal(0, 1, n) * rng.lognormal(0, 2, n) for n in (1, 2, 31, 257, 5000)]
+    cases.append(np.array([2.0, -2.0, 2.0, 1.0, -1.0, 2.0]))     # ties
+    cases.append(inputs.make_config(4).gaussians.s0_jy)          # 25 % negative, 5660 components
+    for w in cases:
+        for f in (0.0, 0.3, 0.5, 0.8, 0.999999, 1.0, 2.0):
+            keep, nk = ctx.truncate_select(torch.as_tensor(w, device="cuda:0"), f)
+            ref = otrunc.keep_mask(w, f)
+            assert np.array_equal(keep.cpu().numpy().astype(bool), ref), (w.size, f)
+            assert int(nk[0]) == int(ref.sum())
+    keep, nk = ctx.truncate_select(torch.zeros(0, dtype=torch.float64, device="cuda:0"), 0.5)
+    assert int(nk[0]) == 0 and keep.numel() == 0
+
+
+@pytest.mark.gpu
+def test_gpu_eq25_basis_sums_match_the_oracle(ctx):
+    # sum_pixels |(G * B_q)| for every basis function: with and without the beam, rotated, rectangular pixels
+    for p_max, beam in ((6, None), (9, (1.5 * ARCMIN, 1.0 * ARCMIN, 0.7, 6)), (20, (1.0 * ARCMIN, 1.0 * ARCMIN, 0.0, 4))):
+        g = (70, 54, -0.4 * ARCMIN, 0.45 * ARCMIN, 0.3 * ARCMIN, -0.2 * ARCMIN)
+        b1, b2, pa = 3.0 * ARCMIN, 2.2 * ARCMIN, 1.2
+        kw = {} if beam is None else dict(bmaj=beam[0], bmin=beam[1], bpa=beam[2], half_width=beam[3])
+        A = shamfi.design_matrix(*g, 0.1 * ARCMIN, 0.0, pa, b1, b2, p_max, **kw)
+        ref = np.abs(A).sum(axis=0)
+        got = ctx.shapelet_basis_sums(*g, 0.1 * ARCMIN, 0.0, pa, p_max, b1, b2, beam=beam).cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-11 * ref.max()
+        coeff = np.arange(1.0, ref.size + 1) * (-1.0) ** np.arange(ref.size)
+        assert np.allclose(np.abs(coeff) * got, shamfi.truncation_weights(coeff, A), rtol=1e-11)
+
+
+@pytest.mark.gpu
+def test_components_and_shapelets_are_truncated_consistently(ctx):
+    from paper_2005_09316_b200 import truncate
     wl = inputs.make_config(4)               # MS-CLEAN-like: 25 % negative components
-    g = truncate.truncate_components(wl.gaussians, 0.5)
+    g = truncate.truncate_components(ctx, wl.gaussians, 0.5)
     assert 0 < g.n < wl.gaussians.n
     assert np.abs(g.s0_jy).min() >= np.sort(np.abs(wl.gaussians.s0_jy))[::-1][g.n - 1] - 1e-15
     assert (g.s0_jy < 0).any() and g.maj_fwhm_rad.shape == g.l.shape == g.pa_rad.shape
     assert np.abs(g.s0_jy).sum() <= 0.5 * np.abs(wl.gaussians.s0_jy).sum() * (1 + 1e-12)
-    full = truncate.truncate_components(wl.points, 1.0)
+    full = truncate.truncate_components(ctx, wl.points, 1.0)
     assert full.n == wl.points.n and np.array_equal(full.l, wl.points.l)
-
-
-def test_shapelet_truncation_keeps_csr_consistent():
-    wl = inputs.make_config(5)
-    s = wl.shapelets
-    w = truncate.shapelet_basis_weights(s)
+    s = inputs.make_config(5).shapelets
+    w = truncate.shapelet_basis_weights(ctx, s)
     assert w.shape == s.coeff.shape and (w >= 0).all() and w.max() > 0
     for f in (1.0, 0.6, 0.2):
-        t = truncate.truncate_shapelets(s, f, w)
+        t = truncate.truncate_shapelets(ctx, s, f, w)
         assert t.coeff_offset[0] == 0 and t.coeff_offset[-1] == t.coeff.size == t.n1.size == t.n2.size
         assert np.all(np.diff(t.coeff_offset) >= 0) and t.n == s.n
         if f == 1.0:
@@ -51,8 +122,8 @@ def test_shapelet_truncation_keeps_csr_consistent():
         else:
             assert 0 < t.coeff.size < s.coeff.size
     empty = inputs.make_config(2).shapelets                      # a config without shapelets passes through
-    assert truncate.truncate_shapelets(empty, 0.5).n == 0
-    # the (0,0) weight is |C| * 1 by construction (pixel-sum normalisation of each component's basis)
+    assert truncate.truncate_shapelets(ctx, empty, 0.5).n == 0
+    # the (0,0) basis image is a unit-sum Gaussian: its Eq 25 weight is |C_00| (to the grid's truncation)
     j0 = int(s.coeff_offset[0])
     assert s.n1[j0] == 0 and s.n2[j0] == 0
-    assert np.isclose(w[j0], abs(s.coeff[j0] * s.s0_jy[0]))
+    assert np.isclose(w[j0], abs(s.coeff[j0] * s.s0_jy[0]), rtol=1e-6)
