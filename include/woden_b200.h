@@ -153,8 +153,8 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n,
 /* Whole-sky convenience call on HOST buffers (the call a user with a sky model in host memory
  * makes; bench.py's end-to-end number).  Every pointer inside the structs and `vis_host` is
  * HOST memory (pinned or pageable).  Copies inputs to the GPU, runs the three predictors above
- * (overwrite, then accumulate), the last of them in up to 8 chunks of time steps whose results
- * are copied back on an internal second stream while the next chunk is computed (pinned
+ * (overwrite, then accumulate), the last of them in up to 8 chunks of time steps (of at least 64 MB of
+ * output each) whose results are copied back on an internal second stream while the next chunk is computed (pinned
  * `vis_host` makes that overlap real), and synchronises both streams before returning.
  * A type with n == 0 may have NULL arrays. */
 typedef struct {

@@ -554,7 +554,12 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     if (last > 0) rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
     if (rc == WODEN_OK && last > 1 && ng > 0)
         rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, 1, st);
-    const int n_chunks = n_times < SIM_CHUNKS ? n_times : SIM_CHUNKS;
+    // chunks of >= 64 MB of output: enough to hide the copy-back, not so many that the last predictor's
+    // launch sequence (staging included) is repeated over small grids
+    int n_chunks = (int)((nvis * 8 + (64u << 20) - 1) / (64u << 20));
+    if (n_chunks > SIM_CHUNKS) n_chunks = SIM_CHUNKS;
+    if (n_chunks > n_times) n_chunks = n_times;
+    if (n_chunks < 1) n_chunks = 1;
     for (int c = 0; c < n_chunks && rc == WODEN_OK; ++c) {
         const int t0 = (int)((long long)n_times * c / n_chunks), t1 = (int)((long long)n_times * (c + 1) / n_chunks);
         woden_uvw part = uvw;
