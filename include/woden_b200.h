@@ -250,8 +250,9 @@ int woden_peel(woden_ctx *ctx, int n_antennas, long long n_cells,
  * DEVICE int[1] or NULL.  n_refine: refinement passes of the normal equations with the exact FP64
  * operator (the tensor-core Gram matrix only preconditions them); 0 selects the default (6), which
  * reaches the FP64 least-squares solution when the scaled design matrix has a condition number
- * below ~10^3 and otherwise still reduces the residual monotonically.  0 <= p_max <= 48
- * (WODEN_ERR_ORDER), half_width <= 24, n_l n_m <= 2^22 (WODEN_ERR_DIM).  A Gram matrix that is not
+ * below ~10^3 and otherwise still reduces the residual monotonically.  0 <= p_max <= 86 (the paper's
+ * orders, :183; WODEN_ERR_ORDER), half_width <= 24, n_l n_m <= 2^22 and P n_l n_m <= 2^32 (the FP64 design
+ * matrix is kept in device memory: WODEN_ERR_DIM).  A Gram matrix that is not
  * positive definite even after diagonal loading is counted for woden_check(). */
 typedef struct {
     int n_l, n_m;
@@ -261,7 +262,7 @@ typedef struct {
     double bmaj_rad, bmin_rad, bpa_rad;
     int half_width;
 } woden_restoring_beam;
-#define WODEN_FIT_MAX_ORDER 48
+#define WODEN_FIT_MAX_ORDER 86
 int woden_fit_shapelets(woden_ctx *ctx, const woden_image_grid *grid, const double *image,
                         double l0, double m0, double pa_rad, int p_max,
                         int n_beta, const double *beta1_rad, const double *beta2_rad,

@@ -33,7 +33,7 @@ WODEN_SHAPELET_REGISTER = 1
 WODEN_SHAPELET_TENSOR = 2
 WODEN_BASIS_RECURRENCE = 0
 WODEN_BASIS_LUT = 1
-WODEN_FIT_MAX_ORDER = 48
+WODEN_FIT_MAX_ORDER = 86
 PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA_IMM": 6, "F2F": 7,
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12, "FFMA2_UR": 13, "WALK": 14}
 

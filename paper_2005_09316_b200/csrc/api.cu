@@ -683,6 +683,7 @@ int fit_setup(woden_ctx *ctx, const woden_image_grid *grid, double l0, double m0
     const int n_pix = grid->n_l * grid->n_m;
     const FitSizes sz = fit_sizes(n_pix, p_max);
     if (full && sz.n_pad > FIT_MAX_N) return WODEN_ERR_ORDER;
+    if (sz.at_doubles > (1ull << 32)) return WODEN_ERR_DIM;             // 32 GB of FP64 design matrix
     const size_t small = (size_t)4 * sz.n_pad + n_pix + 49 * 49 + 64;        // scale, abssum, z, g | r | stencil
     CU(ctx, ctx->f_hx.reserve(sz.hermite_doubles * 8), "alloc fit Hermite tables");
     CU(ctx, ctx->f_at.reserve(sz.at_doubles * 8), "alloc fit design matrix");

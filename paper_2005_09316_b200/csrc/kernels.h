@@ -96,7 +96,7 @@ cudaError_t launch_series(int method, const float *x, const float *c, int PM, lo
                           double dx, float *out, cudaStream_t st);
 
 // ---- image-space shapelet fit (fit.cu) ------------------
-constexpr int FIT_MAX_N = 1280;          // padded unknowns the single-CTA factorisation handles (p_max <= 48)
+constexpr int FIT_MAX_N = 3840;          // padded unknowns (p_max <= 86: 3828): the substitution kernel's shared vector
 struct FitSizes {
     int P, n_rt, n_pad, n_kt, n_pairs, n_split, kt_per_split;
     size_t hermite_doubles, at_doubles, ops_halves, partial_floats, gram_doubles;

@@ -123,6 +123,27 @@ def test_ill_conditioned_fit_matches_in_image_space(ctx):
     assert np.all(np.isfinite(coeff[0]))
 
 
+def test_fit_at_the_orders_of_the_paper(ctx):
+    # p_max = 46 is the paper's phase I order (1128 basis functions); 60 is config 4's.
+    # 9 and 15 row tiles of 128, 18 and 30 Cholesky panels; fitted image and residual against lstsq,
+    # coefficients too when the scaled design matrix is well conditioned.
+    for p_max, n in ((46, 150), (60, 200)):
+        pa, pix = 0.4, 0.3 * ARCMIN
+        g = (n, n, -pix, pix, 0.0, 0.0)
+        beta = n * pix * 2.3548 / (2.0 * 2.5 * np.sqrt(2 * p_max + 1.0))
+        planted = _planted(p_max, p_max, 8.0)
+        rng = np.random.default_rng(p_max)
+        img = shamfi.render(planted, *g, 0.0, 0.0, pa, beta, 0.9 * beta, p_max)
+        img = img + rng.normal(0, 0.01 * np.abs(img).max(), img.shape)
+        x_ref, res_ref, A = shamfi.fit(img, *g, 0.0, 0.0, pa, beta, 0.9 * beta, p_max)
+        coeff, resid, _, _ = _gpu_fit(ctx, img, g, 0.0, 0.0, pa, p_max, [beta], [0.9 * beta])
+        power = float(img.ravel() @ img.ravel())
+        assert np.abs(A @ (coeff[0] - x_ref)).max() <= 1e-8 * np.abs(img).max(), p_max
+        assert abs(resid[0] - res_ref) <= 1e-9 * power, p_max
+        if np.linalg.cond(A / np.abs(A).max(axis=0)) < 1e3:
+            assert np.abs(coeff[0] - x_ref).max() <= 1e-8 * np.abs(x_ref).max(), p_max
+
+
 def test_round_trip_image_to_fit_to_predicted_visibilities(ctx):
     # image of a planted model -> woden_fit_shapelets -> woden_predict_shapelets, against the oracle
     # predicting the PLANTED coefficients (Eq 15-17): north_star tolerance 1e-4 sum|coeff|
@@ -159,7 +180,7 @@ def test_fit_error_codes(ctx):
     from paper_2005_09316_b200 import binding
     img = torch.zeros((16, 16), dtype=torch.float64, device="cuda:0")
     with pytest.raises(binding.WodenError) as e:
-        ctx.fit_shapelets(img, 1e-4, 1e-4, 0, 0, 0, 0, 0.0, 49, [1e-3], [1e-3])
+        ctx.fit_shapelets(img, 1e-4, 1e-4, 0, 0, 0, 0, 0.0, 87, [1e-3], [1e-3])
     assert e.value.status == binding.WODEN_ERR_ORDER
     with pytest.raises(binding.WodenError) as e:
         ctx.fit_shapelets(img, 0.0, 1e-4, 0, 0, 0, 0, 0.0, 4, [1e-3], [1e-3])
