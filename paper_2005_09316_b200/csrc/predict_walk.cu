@@ -27,20 +27,27 @@
 //   The kernel accumulates sum S q with q = exp(+i theta), theta = 2 pi frac(phi);
 //   exp(-2 pi i phi) = conj(q), so the epilogue stores (re, -im).
 //
-// Operand delivery.  The register file of an SM sub-partition feeds about
-// two 32-bit operands per lane per clock, so an FFMA2 with three fresh register pairs costs three
-// cycles instead of two (profiles/pipes_r1.txt).  Everything a component contributes besides the
-// thread's own baseline -- its direction (l, m, n-1), its envelope scales and its 32 fluxes
-// S_k(nu_f) of the channel tile -- is the same for every thread of the launch, so it is served from
-// the CONSTANT BANK: ptxas loads it into uniform registers (SASS LDCU) and the accumulate becomes
-// FFMA2 R, R, UR, R with two register pairs.  There is no shared-memory staging, no barrier and no
-// divergent branch in the kernel.  The price is that the constant bank is fixed per launch: one
-// launch covers one channel tile and one block of <= 204 (186) components (32 KB of the 64 KB
-// bank); the accumulators are carried from launch to launch through the output buffer (a
-// read-modify-write of 8 B per visibility per launch, < 10 % of the launch's duration on
-// HBM and overlapped by the other CTAs).  Launches alternate between the two halves of the bank
-// and between two streams that own disjoint parts of the output, so the copy into one half and the
-// tail of one launch hide behind the launch running from the other half.
+// Operand delivery.  The register file of an SM sub-partition has an even
+// and an odd bank, each feeding one 32-bit operand per lane per clock, and every instruction holds
+// the read stage for max(#even, #odd) distinct registers it reads (operands served by the
+// operand-reuse cache -- same register, same slot, previous instruction -- are free).  Measured on
+// the B200, the kernel's time is 1.05 x the sum of those read cycles over ALL its instructions
+// (profiles/walk_rf_r2.md), not the FMA pipe's 2 cycles per FFMA2.  Hence:
+//   * everything a component contributes besides the thread's own baseline -- its direction
+//     (l, m, n-1), its envelope scales and its 32 fluxes S_k(nu_f) of the channel tile -- is the same
+//     for every thread of the launch and is served from the CONSTANT BANK: ptxas loads it into
+//     uniform registers (SASS LDCU) and the accumulate becomes FFMA2 R, R, UR, R;
+//   * the recurrence is written fma2(y_j, c, y_{j-1}) with the chain value FIRST: ptxas then keeps
+//     y_j in operand slot A of the recurrence (flagged .reuse) and of the accumulate that follows
+//     it, so a (recurrence, accumulate) pair reads 3 + 1 register pairs instead of 3 + 2.
+// There is no shared-memory staging, no barrier and no divergent branch in the kernel.  The price
+// is that the constant bank is fixed per launch: one launch covers one channel tile and one block
+// of <= 204 (186) components (32 KB of the 64 KB bank); the accumulators are carried from launch
+// to launch through the output buffer (a read-modify-write of 8 B per visibility per launch,
+// < 10 % of the launch's duration on HBM and overlapped by the other CTAs).  Launches alternate
+// between the two halves of the bank and between two streams that own disjoint parts of the
+// output, so the copy into one half and the tail of one launch hide behind the launch running
+// from the other half.
 #include <type_traits>
 
 #include "kernels.h"
@@ -98,7 +105,7 @@ struct Seed {
 
 template <bool GAUSS, typename Geo>
 __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, double w, float uf, float vf,
-                                          double sfA, double ds, double magic, int kshift, Seed<GAUSS> &sd)
+                                          double sfA, double ds, double magic, int kshift, float qmax, Seed<GAUSS> &sd)
 {
     // S3: D = u l + v m + w (n-1), FP64 metres
     const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
@@ -119,7 +126,7 @@ __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, doub
         // Eq 13-14 in metres: gx = cg maj (sin pa u + cos pa v), gy = cg min (cos pa u - sin pa v)
         const float gx = fmaf(g.as, uf, g.ac * vf);
         const float gy = fmaf(g.bc, uf, -g.bs * vf);
-        sd.Q = fminf(fmaf(gx, gx, gy * gy), 1.0e30f);     // finite: 0 x inf cannot arise below
+        sd.Q = fminf(fmaf(gx, gx, gy * gy), qmax);        // see EnvConst::qmax: 0 x inf cannot arise below
     } else {
         sd.Q = 0.f;
     }
@@ -129,6 +136,12 @@ __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, doub
 struct EnvConst {
     f32x2 e0, ef, eb;   // xi at J0; forward ratio J0 -> J0+1; backward ratio J0 -> J0-1
     float e2;           // second difference
+    // Largest Q this thread walks with: Q |ef|, Q |eb| <= 126, so every step ratio 2^(Q e) is finite.
+    // Where the clamp bites, xi at J0 is 2^(-126 |e0| / |eb|) with |e0| / |eb| ~ s / (2 ds) >= 32 (the
+    // walking path is only taken when a chain spans at most +-12.5 % in frequency, api.cu): it has
+    // flushed to zero, as has the true envelope at every channel of the chain (< 2^-90), and the chain
+    // is an exact 0 instead of 0 x inf = NaN.  Otherwise the clamp is idle.
+    float qmax;
 };
 
 template <bool GAUSS>
@@ -158,7 +171,7 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     const double magic = magic32_shifted(kshift);
 
     EnvConst ec;
-    ec.e0 = ec.ef = ec.eb = 0ull; ec.e2 = 0.f;
+    ec.e0 = ec.ef = ec.eb = 0ull; ec.e2 = 0.f; ec.qmax = 0.f;
     if constexpr (GAUSS) {
         // exponent(s) = -Q s^2, s_j = s_J0 + (j - J0) ds
         const float e0A = (float)(-sfA * sfA), e0B = (float)(-sfB * sfB);
@@ -166,6 +179,8 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
         const float ebA = (float)(2.0 * sfA * ds - ds * ds), ebB = (float)(2.0 * sfB * ds - ds * ds);
         ec.e0 = pack2(e0A, e0B); ec.ef = pack2(efA, efB); ec.eb = pack2(ebA, ebB);
         ec.e2 = (float)(-2.0 * ds * ds);
+        const float emax = fmaxf(fmaxf(fabsf(efA), fabsf(efB)), fmaxf(fabsf(ebA), fabsf(ebB)));
+        ec.qmax = fminf(126.f / emax, 1.0e30f);
     }
 
     // accumulators: y_j = s_j x_j of q = conj(exp(-2 pi i phi)); the output holds V = (s re, -s im),
@@ -190,12 +205,12 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     }
 
     Seed<GAUSS> sd;
-    make_seed<GAUSS>(rec[k0].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, sd);
+    make_seed<GAUSS>(rec[k0].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, ec.qmax, sd);
 #pragma unroll 2
     for (int k = k0; k < k1; ++k) {
         // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
         Seed<GAUSS> nx;
-        make_seed<GAUSS>(rec[k + 1 < k1 ? k + 1 : k].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, nx);
+        make_seed<GAUSS>(rec[k + 1 < k1 ? k + 1 : k].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, ec.qmax, nx);
 
         // word j = (S[j], S[j + H]), read as 128-bit granules into uniform registers
         const ulonglong2 *fl = rec[k].flux;
@@ -213,15 +228,11 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
             const f32x2 Q2 = pack2(sd.Q, sd.Q);
             unpack2(mul2(Q2, ec.e0), a, b2);
             xb = pack2(ex2_approx(a), ex2_approx(b2));                // xi at J0
-            // The step ratios are clamped to finite values: where xi at J0 has flushed to zero
-            // (Q s^2 > 126) a ratio 2^(+big) would give 0 x inf = NaN; clamped, the chain is an
-            // exact 0, which it is to 2^-90 because the walking path is only taken when a chain
-            // spans at most +-12.5 % in frequency (api.cu).  Where xi at J0 is normal the ratio
-            // exponents are <= 2 x 126 x 1/64 and the clamp is idle.
+            // step ratios: finite because Q <= ec.qmax (see EnvConst)
             unpack2(mul2(Q2, ec.ef), a, b2);
-            rf = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b2, 126.f)));   // xi_{J0+1} / xi_{J0}
+            rf = pack2(ex2_approx(a), ex2_approx(b2));                // xi_{J0+1} / xi_{J0}
             unpack2(mul2(Q2, ec.eb), a, b2);
-            rb = pack2(ex2_approx(fminf(a, 126.f)), ex2_approx(fminf(b2, 126.f)));   // xi_{J0-1} / xi_{J0}
+            rb = pack2(ex2_approx(a), ex2_approx(b2));                // xi_{J0-1} / xi_{J0}
             const float qf = ex2_approx(sd.Q * ec.e2);
             qq = pack2(qf, qf);
             xf = mul2(xb, rf);                                        // xi at J0 + 1
@@ -231,8 +242,7 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
         // ---- both directions in lock step: forward y_{j+1} = (s_{j+1} s_j) c y_j + y_{j-1} over positions
         // J0+1 .. H-1, backward y_{j-1} = (s_{j-1} s_j) c y_j + y_{j+1} over J0 .. 0.  At step t the
         // forward chain sits at jf = J0 + 1 + t and the backward chain at jb = J0 - t; the sign pattern is
-        // symmetric about J0 + 1/2, so the four recurrence FMAs of a step share one scalar (+c or -c):
-        // issued back to back they read it once (operand reuse), see DESIGN.md section 7.
+        // symmetric about J0 + 1/2, so the four recurrence FMAs of a step share one scalar (+c or -c).
         {
             f32x2 fra = r0, fia = i0, frc = r1, fic = i1;      // forward: previous, current
             f32x2 bra = r1, bia = i1, brc = r0, bic = i0;      // backward
@@ -241,22 +251,24 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
                 const int jf = J0 + 1 + t, jb = J0 - t;
                 static_assert(H == 2 * (J0 + 1), "chains are walked symmetrically");
                 f32x2 frn = 0ull, fin = 0ull, brn = 0ull, bin = 0ull;
-                if (t + 1 < H / 2) {
-                    const bool flip = walk_neg(jf + 1) != walk_neg(jf);
-                    const f32x2 cc = flip ? nc2 : c2;           // same for jb - 1 vs jb (symmetry)
-                    frn = fma2(cc, frc, fra); fin = fma2(cc, fic, fia);
-                    brn = fma2(cc, brc, bra); bin = fma2(cc, bic, bia);
-                }
+                const bool more = t + 1 < H / 2;
+                const bool flip = walk_neg(jf + 1) != walk_neg(jf);
+                const f32x2 cc = flip ? nc2 : c2;           // same for jb - 1 vs jb (symmetry)
                 f32x2 Sf = (jf & 1) ? fl[jf >> 1].y : fl[jf >> 1].x;
                 f32x2 Sb = (jb & 1) ? fl[jb >> 1].y : fl[jb >> 1].x;
                 if constexpr (GAUSS) {
                     Sf = mul2(Sf, xf); Sb = mul2(Sb, xb);
-                    if (t + 1 < H / 2) { xf = mul2(xf, rf); rf = mul2(rf, qq); xb = mul2(xb, rb); rb = mul2(rb, qq); }
+                    if (more) { xf = mul2(xf, rf); rf = mul2(rf, qq); xb = mul2(xb, rb); rb = mul2(rb, qq); }
                 }
-                acc_re[jf] = fma2(Sf, frc, acc_re[jf]);
-                acc_im[jf] = fma2(Sf, fic, acc_im[jf]);
-                acc_re[jb] = fma2(Sb, brc, acc_re[jb]);
-                acc_im[jb] = fma2(Sb, bic, acc_im[jb]);
+                // each recurrence is followed by the accumulate of the same chain value (shared operand)
+                if (more) frn = fma2(frc, cc, fra);
+                acc_re[jf] = fma2(frc, Sf, acc_re[jf]);
+                if (more) fin = fma2(fic, cc, fia);
+                acc_im[jf] = fma2(fic, Sf, acc_im[jf]);
+                if (more) brn = fma2(brc, cc, bra);
+                acc_re[jb] = fma2(brc, Sb, acc_re[jb]);
+                if (more) bin = fma2(bic, cc, bia);
+                acc_im[jb] = fma2(bic, Sb, acc_im[jb]);
                 fra = frc; fia = fic; frc = frn; fic = fin;
                 bra = brc; bia = bic; brc = brn; bic = bin;
             }
