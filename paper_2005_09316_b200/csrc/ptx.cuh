@@ -68,6 +68,14 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
 // ---- tcgen05 (5th-generation tensor cores): TMEM allocation, UMMA issue, commit, TMEM loads -----
 namespace woden {
 
+// true in exactly one lane of a converged warp (SASS ELECT): marks single-thread issue regions for ptxas
+__device__ __forceinline__ bool elect_one_sync()
+{
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+    return pred != 0;
+}
+
 // one full warp allocates `ncols` (power of two >= 32) TMEM columns; the base address lands in smem
 __device__ __forceinline__ void tmem_alloc(uint32_t *holder_smem, uint32_t ncols)
 {
