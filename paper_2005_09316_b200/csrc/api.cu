@@ -61,7 +61,7 @@ struct woden_ctx {
 
 namespace {
 
-constexpr int SHAPELET_TENSOR_MIN_ORDER = 40;   // order bucket from which the tensor path measured faster
+constexpr int SHAPELET_TENSOR_MIN_ORDER = 24;   // order bucket from which the tensor path measured faster (profiles/shapelet_mma_r2.md)
 constexpr int SIM_CHUNKS = 8;   // time chunks of woden_simulate_host (compute / copy-back overlap)
 constexpr int CHAN_TILE = 32;   // F_pad granularity: lcm of the kernels' channel tiles
 constexpr int WALK_MIN_F = 8;   // shorter channel lists take the general path
@@ -422,7 +422,7 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     // the kernel variant that skips empty 4-coefficient chunks (decided from the list length alone)
     const bool sparse = (double)n_coeff < 0.75 * (double)n * (double)((PM + 1) * (PM + 2) / 2);
     // tensor-core variant (north_star: "used only if ... shown by measurement to beat the register path"):
-    // AUTO takes it from the order bucket at which it measured faster (profiles/shapelet_mma_r1.md)
+    // AUTO takes it from the order bucket at which it measured faster (profiles/shapelet_mma_r2.md)
     const bool tensor = ctx->shapelet_path == WODEN_SHAPELET_TENSOR ||
                         (ctx->shapelet_path == WODEN_SHAPELET_AUTO && PM >= SHAPELET_TENSOR_MIN_ORDER);
     if (tensor) {
