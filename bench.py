@@ -41,8 +41,8 @@ SM_MAX_HZ = 1965e6
 # from the ncu --set full captures summarised in profiles/ncu_r2_kernels.md (not measured in this run):
 # (component type, path) -> (kernel, bytes, commit the capture was taken at)
 NCU_DRAM_BYTES = {
-    ("points", "walk"): ("predict_walk_kernel<false>", 10982400 + 71157248, "fcd6054"),
-    ("gaussians", "walk"): ("predict_walk_kernel<true>", 10996992 + 75553536, "fcd6054"),
+    ("points", "walk"): ("predict_walk_kernel<false>", 10981376 + 70713088, "4acabf5"),
+    ("gaussians", "walk"): ("predict_walk_kernel<true>", 10989312 + 76573952, "4acabf5"),
 }
 KERNEL_NAMES = {("points", "walk"): "predict_walk_kernel<false>", ("gaussians", "walk"): "predict_walk_kernel<true>",
                 ("points", "general"): "predict_pg_kernel<16, false>", ("gaussians", "general"): "predict_pg_kernel<16, true>",
