@@ -550,10 +550,18 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     // All types but the last run over the whole observation in one launch (no tail loss); only
     // the last one is chunked, and its chunks' copies hide behind the chunks that follow.
     const int last = ns > 0 ? 2 : (ng > 0 ? 1 : 0);
+    // The first non-empty type overwrites the buffer, the others accumulate (no zero-fill pass, no
+    // read-modify-write where there is nothing to add to).
     int rc = WODEN_OK;
-    if (last > 0) rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
-    if (rc == WODEN_OK && last > 1 && ng > 0)
-        rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, 1, st);
+    int written = 0;
+    if (last > 0 && np > 0) {
+        rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
+        written = 1;
+    }
+    if (rc == WODEN_OK && last > 1 && ng > 0) {
+        rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, written, st);
+        written = 1;
+    }
     // chunks of >= 64 MB of output: enough to hide the copy-back, not so many that the last predictor's
     // launch sequence (staging included) is repeated over small grids
     int n_chunks = (int)((nvis * 8 + (64u << 20) - 1) / (64u << 20));
@@ -572,10 +580,10 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
         if (last == 0)
             rc = woden_predict_points(ctx, &part, np, pl, pm, ps, pa, ref_freq_hz, vc, 0, st);
         else if (last == 1)
-            rc = woden_predict_gaussians(ctx, &part, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vc, 1, st);
+            rc = woden_predict_gaussians(ctx, &part, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vc, written, st);
         else
             rc = woden_predict_shapelets(ctx, &part, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
-                                         shp->p_max, sn1, sn2, sc, vc, 1, st);
+                                         shp->p_max, sn1, sn2, sc, vc, written, st);
         if (rc != WODEN_OK) break;
         CU(ctx, cudaEventRecord(ctx->chunk_done[c], st), "record chunk");
         CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->chunk_done[c], 0), "wait chunk");
