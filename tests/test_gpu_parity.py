@@ -342,6 +342,45 @@ def test_accumulate_zero_components_and_additivity(ctx, torch_mod):
     assert torch.equal(again, total)
 
 
+@pytest.mark.parametrize("keep", ["points", "gaussians", "shapelets", "gaussians+shapelets", "none"])
+def test_first_non_empty_type_overwrites_a_dirty_buffer(ctx, torch_mod, keep):
+    """DeviceWorkload.predict and woden_simulate_host let the first non-empty component type overwrite the buffer
+    (no zero-fill pass): whatever the buffer held before, the result is the sum of the types present."""
+    from paper_2005_09316_b200 import binding
+    torch = torch_mod
+    ctx.set_path(0)
+    wl = inputs.make_config(1)
+    full = binding.DeviceWorkload(wl, ctx=ctx)
+    dw = binding.DeviceWorkload(wl, ctx=ctx)
+    if "points" not in keep: dw.p = None
+    if "gaussians" not in keep: dw.g = None
+    if "shapelets" not in keep: dw.s = None
+    # reference: each present type alone into zeros, summed
+    ref = torch.zeros(full.uvw.vis_shape, dtype=torch.complex64, device="cuda:0")
+    if dw.p is not None:
+        ctx.predict_points(full.uvw, *full.p, wl.ref_freq_hz, ref, accumulate=True)
+    if dw.g is not None:
+        l, m, s0, al, mj, mn, pa = full.g
+        ctx.predict_gaussians(full.uvw, l, m, s0, al, wl.ref_freq_hz, mj, mn, pa, ref, accumulate=True)
+    if dw.s is not None:
+        l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = full.s
+        ctx.predict_shapelets(full.uvw, l, m, s0, al, wl.ref_freq_hz, b1, b2, pa, M, off, nc, pmax, n1, n2, cf, ref, True)
+    dirty = torch.full(full.uvw.vis_shape, float("nan"), dtype=torch.complex64, device="cuda:0")
+    out = dw.predict(ctx, vis=dirty)
+    torch.cuda.synchronize()
+    assert torch.all(torch.isfinite(torch.view_as_real(out)))
+    assert torch.max(torch.abs(out - ref)).item() < 2e-5
+    if keep == "none":
+        assert torch.all(out == 0)
+    # the same through woden_simulate_host (its device buffer is whatever the previous call left there)
+    if "points" not in keep: wl.points = inputs.empty_components()
+    if "gaussians" not in keep: wl.gaussians = inputs.empty_components()
+    if "shapelets" not in keep: wl.shapelets = inputs.empty_components()
+    host = np.full((wl.n_times, wl.n_freqs, wl.n_baselines), np.nan, dtype=np.complex64)
+    ctx.simulate_host(wl, host)
+    assert np.array_equal(host, out.cpu().numpy())
+
+
 def test_phase_centre_point_and_hermitian_symmetry_on_gpu(ctx, torch_mod):
     from paper_2005_09316_b200 import binding
     torch = torch_mod
