@@ -3,9 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5]
 
-One "step" = one pass of the whole hot path over one workload: woden_predict_points
-(overwrite), woden_predict_gaussians and woden_predict_shapelets (accumulate; the first non-empty type
-overwrites) on config 5
+One "step" = one pass of the whole hot path over one workload: woden_predict_shapelets,
+woden_predict_points and woden_predict_gaussians (the first non-empty type overwrites the
+buffer, the others accumulate) on config 5
 ("Full-band mixed sky", the largest BASELINE.json config; 1.75e8 visibilities, 8000 points,
 2000 Gaussians, 4 shapelets of 861 coefficients), inputs resident in HBM.  Prints ONE JSON
 line (rank 0).  See DESIGN.md "Measurement" for the definitions of every field.
@@ -272,20 +272,21 @@ def run_ours(args):
     def step(record):
         marks = [ev() for _ in range(4)]
         marks[0].record()
-        # the first non-empty component type overwrites vis, the others accumulate (as DeviceWorkload.predict)
+        # shapelets, points, Gaussians (the order of DeviceWorkload.predict and woden_simulate_host); the first
+        # non-empty component type overwrites vis, the others accumulate
         written = False
-        if dw.p is not None:
-            ctx.predict_points(dw.uvw, *dw.p, dw.ref, vis, False)
+        if dw.s is not None:
+            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = dw.s
+            ctx.predict_shapelets(dw.uvw, l, m, s0, al, dw.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf, vis, False)
             written = True
         marks[1].record()
+        if dw.p is not None:
+            ctx.predict_points(dw.uvw, *dw.p, dw.ref, vis, written)
+            written = True
+        marks[2].record()
         if dw.g is not None:
             l, m, s0, al, mj, mn, pa = dw.g
             ctx.predict_gaussians(dw.uvw, l, m, s0, al, dw.ref, mj, mn, pa, vis, written)
-            written = True
-        marks[2].record()
-        if dw.s is not None:
-            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = dw.s
-            ctx.predict_shapelets(dw.uvw, l, m, s0, al, dw.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf, vis, written)
             written = True
         if not written:
             ctx.predict_points(dw.uvw, None, None, None, None, dw.ref, vis, False)
@@ -312,7 +313,7 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else {}
     ms_total = e0.elapsed_time(e1)
     for marks in recs:
-        for name, a, b in (("points", 0, 1), ("gaussians", 1, 2), ("shapelets", 2, 3)):
+        for name, a, b in (("shapelets", 0, 1), ("points", 1, 2), ("gaussians", 2, 3)):
             per_type_ms[name].append(marks[a].elapsed_time(marks[b]))
     ctx.check()
     ms_total = parallel.max_over_ranks(ms_total, dist, f"cuda:{local}")

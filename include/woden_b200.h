@@ -152,10 +152,13 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n,
 
 /* Whole-sky convenience call on HOST buffers (the call a user with a sky model in host memory
  * makes; bench.py's end-to-end number).  Every pointer inside the structs and `vis_host` is
- * HOST memory (pinned or pageable).  Copies inputs to the GPU, runs the three predictors above
- * (overwrite, then accumulate), the last of them in up to 8 chunks of time steps (of at least 64 MB of
- * output each) whose results are copied back on an internal second stream while the next chunk is computed (pinned
- * `vis_host` makes that overlap real), and synchronises both streams before returning.
+ * HOST memory (pinned or pageable).  Copies inputs to the GPU, runs the three predictors above in the order
+ * shapelets, points, Gaussians (the first non-empty type overwrites, the others accumulate) and copies the result
+ * back on an internal second stream while the LAST predictor is still running (pinned `vis_host` makes that overlap
+ * real): on the channel-walking path that predictor finishes the output one 32-channel tile at a time and every
+ * finished tile is copied back (a strided 2-D copy) under the tiles that follow; otherwise it runs in up to 8 chunks
+ * of time steps (of at least 64 MB of output each) and every finished chunk is copied back under the next one.  Both
+ * streams are synchronised before returning.  The values are bit-identical to the three device calls in that order.
  * A type with n == 0 may have NULL arrays. */
 typedef struct {
     int n;

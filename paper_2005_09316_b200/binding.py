@@ -448,21 +448,23 @@ class DeviceWorkload:
             self.s = None
 
     def predict(self, ctx: Woden, vis=None, stream=None):
-        """The whole hot path: the first non-empty component type overwrites `vis`, the others accumulate."""
+        """The whole hot path in the order shapelets, points, Gaussians (the order woden_simulate_host uses: the
+        longest walking call comes last and hides the copy-back); the first non-empty component type overwrites
+        `vis`, the others accumulate."""
         if vis is None:
             vis = ctx.new_vis(self.uvw)
         written = False
+        if self.s is not None:
+            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = self.s
+            ctx.predict_shapelets(self.uvw, l, m, s0, al, self.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf,
+                                  vis, False, stream)
+            written = True
         if self.p is not None:
-            ctx.predict_points(self.uvw, *self.p, self.ref, vis, False, stream)
+            ctx.predict_points(self.uvw, *self.p, self.ref, vis, written, stream)
             written = True
         if self.g is not None:
             l, m, s0, al, mj, mn, pa = self.g
             ctx.predict_gaussians(self.uvw, l, m, s0, al, self.ref, mj, mn, pa, vis, written, stream)
-            written = True
-        if self.s is not None:
-            l, m, s0, al, b1, b2, pa, M, off, nc, pmax, n1, n2, cf = self.s
-            ctx.predict_shapelets(self.uvw, l, m, s0, al, self.ref, b1, b2, pa, M, off, nc, pmax, n1, n2, cf,
-                                  vis, written, stream)
             written = True
         if not written:         # no components at all: the library zero-fills on an empty overwrite call
             ctx.predict_points(self.uvw, None, None, None, None, self.ref, vis, False, stream)

@@ -50,6 +50,9 @@ struct woden_ctx {
     std::vector<double> chan_s_host;     // nu_f / c of the padded channel list (host copy)
     cudaStream_t walk_stream = nullptr;  // second lane of the channel-walking launches
     cudaEvent_t walk_fork = nullptr, walk_join = nullptr;
+    void (*walk_tile_done)(void *, int, cudaStream_t) = nullptr;   // set by woden_simulate_host around its last call
+    void *walk_tile_user = nullptr;
+    std::vector<cudaEvent_t> tile_events;
     cudaEvent_t fit_t0 = nullptr, fit_t1 = nullptr;   // around the last fit's Gram kernel
     int chan_F_pad = 0;
     ChanTable ch{};
@@ -236,6 +239,7 @@ int woden_destroy(woden_ctx *ctx)
         if (ctx->copy_stream) {
             cudaStreamDestroy(ctx->copy_stream);
             for (cudaEvent_t ev : ctx->chunk_done) if (ev) cudaEventDestroy(ev);
+            for (cudaEvent_t ev : ctx->tile_events) cudaEventDestroy(ev);
         }
         for (DevBuf *b : {&ctx->geo, &ctx->flux, &ctx->tri, &ctx->chan, &ctx->err, &ctx->hang, &ctx->bmat, &ctx->bscale, &ctx->lut, &ctx->wblocks, &ctx->f_hx, &ctx->f_a0, &ctx->f_at, &ctx->f_small, &ctx->f_gram, &ctx->f_ops,
                           &ctx->f_part, &ctx->h_uvw, &ctx->h_comp,
@@ -325,7 +329,7 @@ int woden_predict_points(woden_ctx *ctx, const woden_uvw *uvw, int n, const doub
         unsigned char *blocks = static_cast<unsigned char *>(ctx->wblocks.p);
         launch_pack_walk_points(geo, s0_jy, alpha, ref_freq_hz, n, ctx->ch, blocks, err, st);
         CU(ctx, cudaGetLastError(), "pack points");
-        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join};
+        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join, ctx->walk_tile_done, ctx->walk_tile_user};
         CU(ctx, launch_walk_points(d, ctx->ch, blocks, n, out, accumulate ? 1 : 0, err, ws), "predict_points launch");
         return WODEN_OK;
     }
@@ -370,7 +374,7 @@ int woden_predict_gaussians(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
         unsigned char *blocks = static_cast<unsigned char *>(ctx->wblocks.p);
         launch_pack_walk_gaussians(geo, s0_jy, alpha, ref_freq_hz, n, ctx->ch, blocks, err, st);
         CU(ctx, cudaGetLastError(), "pack gaussians");
-        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join};
+        const WalkStreams ws{st, ctx->walk_stream, ctx->walk_fork, ctx->walk_join, ctx->walk_tile_done, ctx->walk_tile_user};
         CU(ctx, launch_walk_gaussians(d, ctx->ch, blocks, n, out, accumulate ? 1 : 0, err, ws),
            "predict_gaussians launch");
         return WODEN_OK;
@@ -541,54 +545,98 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     }
     if (e != cudaSuccess) return fail_cuda(ctx, e, "host->device copies");
 
-    // Time steps are independent (Eq 9 sums over components only): the last predictor runs in chunks
-    // of time steps and each finished chunk is copied back on a second stream meanwhile.
+    // Order of the three types: shapelets (overwrite), points, Gaussians -- the first non-empty type overwrites
+    // the buffer, the others accumulate.  The device-to-host copy (PCIe: ~28 ms for config 5's 1.4 GB) hides
+    // behind the LAST predictor:
+    //  * channel-walking path, >= 2 channel tiles: the last type (Gaussians, else points) finishes the
+    //    output one 32-channel tile at a time; each finished tile is copied back (a strided 2-D copy) on a
+    //    second stream while the following tiles are computed.  Only the last tile's copy is exposed.
+    //  * otherwise: time steps are independent (Eq 9 sums over components only), so the last predictor runs in
+    //    chunks of time steps and each finished chunk is copied back meanwhile.
     if (!ctx->copy_stream) {
         CU(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking), "create copy stream");
         for (cudaEvent_t &ev : ctx->chunk_done) CU(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "create event");
     }
-    // All types but the last run over the whole observation in one launch (no tail loss); only
-    // the last one is chunked, and its chunks' copies hide behind the chunks that follow.
-    const int last = ns > 0 ? 2 : (ng > 0 ? 1 : 0);
-    // The first non-empty type overwrites the buffer, the others accumulate (no zero-fill pass, no
-    // read-modify-write where there is nothing to add to).
-    int rc = WODEN_OK;
+    int rc = ensure_chan(ctx, &uvw, st);
+    if (rc != WODEN_OK) return rc;
+    const int last = ng > 0 ? 1 : (np > 0 ? 0 : (ns > 0 ? 2 : 0));     // 0 points, 1 Gaussians, 2 shapelets
+    const int n_ftiles = ctx->ch.F_pad / WALK_FT;
+    const bool by_tile = last != 2 && ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform && n_ftiles >= 2;
     int written = 0;
-    if (last > 0 && np > 0) {
-        rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, 0, st);
+    if (last != 2 && ns > 0) {
+        rc = woden_predict_shapelets(ctx, &uvw, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
+                                     shp->p_max, sn1, sn2, sc, vis, 0, st);
         written = 1;
     }
-    if (rc == WODEN_OK && last > 1 && ng > 0) {
-        rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, written, st);
+    if (rc == WODEN_OK && last == 1 && np > 0) {
+        rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, written, st);
         written = 1;
     }
-    // chunks of >= 64 MB of output: enough to hide the copy-back, not so many that the last predictor's
-    // launch sequence (staging included) is repeated over small grids
-    int n_chunks = (int)((nvis * 8 + (64u << 20) - 1) / (64u << 20));
-    if (n_chunks > SIM_CHUNKS) n_chunks = SIM_CHUNKS;
-    if (n_chunks > n_times) n_chunks = n_times;
-    if (n_chunks < 1) n_chunks = 1;
-    for (int c = 0; c < n_chunks && rc == WODEN_OK; ++c) {
-        const int t0 = (int)((long long)n_times * c / n_chunks), t1 = (int)((long long)n_times * (c + 1) / n_chunks);
-        woden_uvw part = uvw;
-        part.n_times = t1 - t0;
-        part.u_m = uvw.u_m + (size_t)t0 * n_baselines;
-        part.v_m = uvw.v_m + (size_t)t0 * n_baselines;
-        part.w_m = uvw.w_m + (size_t)t0 * n_baselines;
-        const size_t off = (size_t)t0 * n_freqs * n_baselines, cnt = (size_t)(t1 - t0) * n_freqs * n_baselines;
-        float *vc = vis + 2 * off;
-        if (last == 0)
-            rc = woden_predict_points(ctx, &part, np, pl, pm, ps, pa, ref_freq_hz, vc, 0, st);
-        else if (last == 1)
-            rc = woden_predict_gaussians(ctx, &part, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vc, written, st);
+    if (rc == WODEN_OK && by_tile) {
+        struct TileCopy {
+            woden_ctx *ctx; const float *vis; float *vis_host; int T, F, B; cudaError_t err; int calls;
+        } tc{ctx, vis, vis_host, n_times, n_freqs, n_baselines, cudaSuccess, 0};
+        while ((int)ctx->tile_events.size() < n_ftiles) {
+            cudaEvent_t ev;
+            CU(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "create event");
+            ctx->tile_events.push_back(ev);
+        }
+        ctx->walk_tile_user = &tc;
+        ctx->walk_tile_done = [](void *user, int ftile, cudaStream_t s) {
+            TileCopy *t = static_cast<TileCopy *>(user);
+            ++t->calls;
+            const int f0 = ftile * WALK_FT, nf = t->F - f0 < WALK_FT ? t->F - f0 : WALK_FT;
+            if (nf <= 0 || t->err != cudaSuccess) return;
+            cudaEvent_t ev = t->ctx->tile_events[ftile];
+            cudaError_t e = cudaEventRecord(ev, s);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(t->ctx->copy_stream, ev, 0);
+            const size_t pitch = (size_t)t->F * t->B * 8, off = (size_t)f0 * t->B * 2;
+            if (e == cudaSuccess)
+                e = cudaMemcpy2DAsync(t->vis_host + off, pitch, t->vis + off, pitch, (size_t)nf * t->B * 8, t->T,
+                                      cudaMemcpyDeviceToHost, t->ctx->copy_stream);
+            t->err = e;
+        };
+        if (last == 1)
+            rc = woden_predict_gaussians(ctx, &uvw, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vis, written, st);
         else
-            rc = woden_predict_shapelets(ctx, &part, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
-                                         shp->p_max, sn1, sn2, sc, vc, written, st);
-        if (rc != WODEN_OK) break;
-        CU(ctx, cudaEventRecord(ctx->chunk_done[c], st), "record chunk");
-        CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->chunk_done[c], 0), "wait chunk");
-        CU(ctx, cudaMemcpyAsync(vis_host + 2 * off, vc, cnt * 8, cudaMemcpyDeviceToHost, ctx->copy_stream),
-           "device->host vis");
+            rc = woden_predict_points(ctx, &uvw, np, pl, pm, ps, pa, ref_freq_hz, vis, written, st);
+        ctx->walk_tile_done = nullptr;
+        ctx->walk_tile_user = nullptr;
+        if (rc == WODEN_OK && tc.err != cudaSuccess) rc = fail_cuda(ctx, tc.err, "device->host vis (tile)");
+        if (rc == WODEN_OK && tc.calls != n_ftiles) {      // the call did not take the tile-wise path after all
+            CU(ctx, cudaEventRecord(ctx->chunk_done[0], st), "record");
+            CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->chunk_done[0], 0), "wait");
+            CU(ctx, cudaMemcpyAsync(vis_host, vis, nvis * 8, cudaMemcpyDeviceToHost, ctx->copy_stream), "device->host vis");
+        }
+    } else if (rc == WODEN_OK) {
+        // chunks of >= 64 MB of output: enough to hide the copy-back, not so many that the last predictor's
+        // launch sequence (staging included) is repeated over small grids
+        int n_chunks = (int)((nvis * 8 + (64u << 20) - 1) / (64u << 20));
+        if (n_chunks > SIM_CHUNKS) n_chunks = SIM_CHUNKS;
+        if (n_chunks > n_times) n_chunks = n_times;
+        if (n_chunks < 1) n_chunks = 1;
+        for (int c = 0; c < n_chunks && rc == WODEN_OK; ++c) {
+            const int t0 = (int)((long long)n_times * c / n_chunks), t1 = (int)((long long)n_times * (c + 1) / n_chunks);
+            woden_uvw part = uvw;
+            part.n_times = t1 - t0;
+            part.u_m = uvw.u_m + (size_t)t0 * n_baselines;
+            part.v_m = uvw.v_m + (size_t)t0 * n_baselines;
+            part.w_m = uvw.w_m + (size_t)t0 * n_baselines;
+            const size_t off = (size_t)t0 * n_freqs * n_baselines, cnt = (size_t)(t1 - t0) * n_freqs * n_baselines;
+            float *vc = vis + 2 * off;
+            if (last == 0)
+                rc = woden_predict_points(ctx, &part, np, pl, pm, ps, pa, ref_freq_hz, vc, written, st);
+            else if (last == 1)
+                rc = woden_predict_gaussians(ctx, &part, ng, gl, gm, gs, ga, ref_freq_hz, gmj, gmn, gpa, vc, written, st);
+            else
+                rc = woden_predict_shapelets(ctx, &part, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,
+                                             shp ? shp->p_max : 0, sn1, sn2, sc, vc, 0, st);
+            if (rc != WODEN_OK) break;
+            CU(ctx, cudaEventRecord(ctx->chunk_done[c], st), "record chunk");
+            CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->chunk_done[c], 0), "wait chunk");
+            CU(ctx, cudaMemcpyAsync(vis_host + 2 * off, vc, cnt * 8, cudaMemcpyDeviceToHost, ctx->copy_stream),
+               "device->host vis");
+        }
     }
     if (rc != WODEN_OK) { cudaStreamSynchronize(st); cudaStreamSynchronize(ctx->copy_stream); return rc; }
     CU(ctx, cudaStreamSynchronize(st), "simulate sync");

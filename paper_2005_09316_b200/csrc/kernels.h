@@ -54,6 +54,10 @@ constexpr int WALK_KC_GAUSS = WALK_CB_BYTES / (48 + WALK_FT * 4);      // 186
 struct WalkStreams {
     cudaStream_t main, aux;      // the caller's stream and the context's second lane
     cudaEvent_t fork, join;
+    // Optional host hook, called right after the last launch of channel tile `ftile` has been enqueued on `st`
+    // (calls with >= 2 channel tiles only): woden_simulate_host starts the copy-back of the finished tile from it.
+    void (*tile_done)(void *user, int ftile, cudaStream_t st) = nullptr;
+    void *user = nullptr;
 };
 size_t walk_blocks_bytes(int n, int n_ftiles, bool gauss);
 void launch_pack_walk_points(const GeoP *geo, const double *s0, const double *alpha, double ref_freq, int n,

@@ -360,6 +360,7 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *
             predict_walk_kernel<GAUSS><<<grid, WTHREADS, 0, st>>>(p); note_launch();
             e = cudaGetLastError();
         }
+        if (e == cudaSuccess && n_ftiles >= 2 && ws.tile_done) ws.tile_done(ws.user, ftile, st);
     }
     // join even after an error so that the caller's stream stays ordered after the aux work
     cudaError_t e2 = cudaEventRecord(ws.join, ws.aux);

@@ -411,31 +411,44 @@ def test_simulate_host_matches_device_path(ctx):
     assert np.array_equal(out, dev)
 
 
+@pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
 @pytest.mark.parametrize("last", ["shapelets", "gaussians", "points"])
-def test_simulate_host_time_chunks_are_bit_identical(ctx, torch_mod, last):
-    # woden_simulate_host runs its LAST predictor in chunks of time steps of >= 64 MB of output: 7 steps
-    # of config 5's grid are 175 MB -> 3 ragged chunks (2, 2, 3 steps).  Whichever component type comes
-    # last (tensor shapelet engine, walking Gaussians, walking points), the chunked result must equal
-    # the one-launch device path bit for bit, and the oracle on a sampled subset.
+def test_simulate_host_overlapped_copy_back_is_bit_identical(ctx, torch_mod, last, path):
+    # woden_simulate_host hides the copy-back behind its LAST predictor (Gaussians, else points, else shapelets):
+    # on the channel-walking path tile by tile (12 channel tiles here, strided 2-D copies), on the general path
+    # and for a shapelet-only sky in chunks of time steps of >= 64 MB of output (7 steps of config 5's grid are
+    # 175 MB -> 3 ragged chunks of 2, 2, 3 steps).  Either way the result must equal the device path (the three
+    # calls in the same order) bit for bit, and the oracle on a sampled subset.
     import dataclasses
     wl = inputs.make_config(5, n_times=7, n_times_total=7)
     keep = lambda c, n: type(c)(**{f.name: (None if getattr(c, f.name) is None else getattr(c, f.name)[:n])
                                    for f in dataclasses.fields(c)})
-    wl.points = keep(wl.points, 300)
-    wl.gaussians = keep(wl.gaussians, 200) if last != "points" else inputs.empty_components()
-    if last != "shapelets":
-        wl.shapelets = inputs.empty_components()
-    ctx.set_path(0)
-    out = np.empty((wl.n_times, wl.n_freqs, wl.n_baselines), dtype=np.complex64)
+    wl.points = keep(wl.points, 300) if last != "shapelets" else inputs.empty_components()
+    wl.gaussians = keep(wl.gaussians, 200) if last == "gaussians" else inputs.empty_components()
+    ctx.set_path(path)
+    out = np.full((wl.n_times, wl.n_freqs, wl.n_baselines), np.nan, dtype=np.complex64)
     assert out.nbytes > 2 * (64 << 20)
     ctx.simulate_host(wl, out)
-    dev = _gpu_total(ctx, wl, 0)
+    dev = _gpu_total(ctx, wl, path)
     assert np.array_equal(out, dev)
     rng = np.random.default_rng(12)
     idx = np.unique(np.concatenate([rng.integers(0, wl.n_vis, 4000), [0, wl.n_vis - 1]])).astype(np.int64)
     ref = oracle.predict_workload(wl, vis_index=idx)
     scale = oracle.workload_tolerance_scale(wl)
     _assert_parity(out.reshape(-1)[idx], ref, scale, idx, wl, "simulate_host")
+
+
+def test_simulate_host_ragged_last_channel_tile(ctx, torch_mod):
+    # tile-wise copy-back with a ragged last tile (F = 75: tiles of 32, 32, 11 channels) and a pageable host buffer
+    u, v, w, fr = _small_case(seed=5, T=3, B=300, F=75, uniform=True)
+    wl = inputs.make_config(1)
+    wl.u_m, wl.v_m, wl.w_m, wl.freqs_hz = u, v, w, fr
+    wl.shapelets = inputs.empty_components()
+    ctx.set_path(0)
+    out = np.full((wl.n_times, wl.n_freqs, wl.n_baselines), np.nan, dtype=np.complex64)
+    ctx.simulate_host(wl, out)
+    dev = _gpu_total(ctx, wl, 0)
+    assert np.array_equal(out, dev)
 
 
 def test_uvw_and_uv_basis_on_device_match_the_oracle(ctx, torch_mod):
