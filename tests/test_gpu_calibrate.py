@@ -23,7 +23,7 @@ def _dev(a):
     return torch.as_tensor(np.ascontiguousarray(a), device="cuda:0")
 
 
-@pytest.mark.parametrize("n_ant", [2, 3, 9, 33, 64])
+@pytest.mark.parametrize("n_ant", [2, 3, 9, 33, 64, 65, 100, 128])      # 65-128: the register-resident kernel
 def test_gains_match_the_oracle_on_random_cells(ctx, n_ant):
     import torch
     rng = np.random.default_rng(n_ant)
