@@ -378,7 +378,7 @@ def run_ours(args):
     basis, peak = ops["walk" if walk else "general"]
     ach = (per_type[dominant]["coeff_evals_per_s"] if dominant == "shapelets"
            else per_type[dominant]["evals_per_s"])
-    # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r1_kernels.md):
+    # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r2_kernels.md):
     # the visibility buffer once, plus the component blocks that miss L2
     key = (dominant, "walk" if walk else "general")
     rec_traffic = NCU_DRAM_BYTES.get(key) if args.config == 5 else None
@@ -396,9 +396,15 @@ def run_ours(args):
         "operand_delivery": {"ffma2_three_fresh_pairs_fma_per_s": ffma2_3reg, "ffma_reused_operands_fma_per_s": fma_rate,
                              "walk_pattern_fma_per_s": walk_rate,
                              "frac_of_walk_pattern": (ach * 4.0 / walk_rate) if (walk and dominant == "points") else None,
-                             "note": "register file feeds ~2 operands/clk/sub-partition: an FMA with three fresh "
-                                     "register operands runs at 2/3 of the pipe rate; the walking kernel's own "
-                                     "4-FFMA2 pattern in isolation sustains walk_pattern_fma_per_s (DESIGN.md section 7)"},
+                             "read_cycle_model": {"pipe_cycles_per_two_components": 271, "read_cycles_final_build": 334,
+                                                  "read_cycles_floor": 317, "measured_over_model": 1.05,
+                                                  "source": "profiles/walk_rf_r2.md (counted on the SASS of the "
+                                                            "committed build; recorded, not measured in this run)"},
+                             "note": "each register bank (even / odd) feeds one operand per lane per clock: an FMA with "
+                                     "three fresh register operands runs at 2/3 of the pipe rate, and the walking "
+                                     "kernel's time is 1.05 x the sum of its instructions' register-read cycles "
+                                     "(profiles/walk_rf_r2.md); its own 4-FFMA2 pattern in isolation sustains "
+                                     "walk_pattern_fma_per_s (DESIGN.md section 7)"},
         "peak_basis": basis + f"; pipe rate measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
         "nominal_mufu_roofline_gevals": SM_COUNT * MUFU_LANES_PER_SM * SM_MAX_HZ / (2 if dominant == "points" else 3) / 1e9,
     }
