@@ -155,8 +155,9 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n,
  * HOST memory (pinned or pageable).  Copies inputs to the GPU, runs the three predictors above in the order
  * shapelets, points, Gaussians (the first non-empty type overwrites, the others accumulate) and copies the result
  * back on an internal second stream while the LAST predictor is still running (pinned `vis_host` makes that overlap
- * real): on the channel-walking path that predictor finishes the output one 32-channel tile at a time and every
- * finished tile is copied back (a strided 2-D copy) under the tiles that follow; otherwise it runs in up to 8 chunks
+ * real): on the channel-walking path, into a page-locked buffer, that predictor finishes the output one 32-channel
+ * tile at a time and every finished tile is copied back (a strided 2-D copy) under the tiles that follow; otherwise
+ * (general path, shapelet-only sky, pageable `vis_host`) it runs in up to 8 chunks
  * of time steps (of at least 64 MB of output each) and every finished chunk is copied back under the next one.  Both
  * streams are synchronised before returning.  The values are bit-identical to the three device calls in that order.
  * A type with n == 0 may have NULL arrays. */

@@ -561,7 +561,12 @@ int woden_simulate_host(woden_ctx *ctx, int n_baselines, int n_times, int n_freq
     if (rc != WODEN_OK) return rc;
     const int last = ng > 0 ? 1 : (np > 0 ? 0 : (ns > 0 ? 2 : 0));     // 0 points, 1 Gaussians, 2 shapelets
     const int n_ftiles = ctx->ch.F_pad / WALK_FT;
-    const bool by_tile = last != 2 && ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform && n_ftiles >= 2;
+    // a copy into pageable memory blocks the HOST until it is done: issued from the launch loop it would starve the
+    // GPU of the launches that follow, so only page-locked buffers take the tile-wise path
+    cudaPointerAttributes attr;
+    const bool pinned = cudaPointerGetAttributes(&attr, vis_host) == cudaSuccess && attr.type == cudaMemoryTypeHost;
+    cudaGetLastError();
+    const bool by_tile = pinned && last != 2 && ctx->path == WODEN_PATH_AUTO && ctx->ch.uniform && n_ftiles >= 2;
     int written = 0;
     if (last != 2 && ns > 0) {
         rc = woden_predict_shapelets(ctx, &uvw, ns, sl, sm, ss, sa, ref_freq_hz, sb1, sb2, spa, sM, so, (int)nc,

@@ -411,14 +411,27 @@ def test_simulate_host_matches_device_path(ctx):
     assert np.array_equal(out, dev)
 
 
+def _host_vis(torch, wl, pinned):
+    """NaN-filled complex64 host buffer [T][F][B]; page-locked (the tile-wise copy-back needs it) or pageable."""
+    shape = (wl.n_times, wl.n_freqs, wl.n_baselines)
+    if pinned:
+        t = torch.empty(shape, dtype=torch.complex64, pin_memory=True)
+        out = t.numpy()
+        out[...] = np.nan
+        return out, t
+    return np.full(shape, np.nan, dtype=np.complex64), None
+
+
+@pytest.mark.parametrize("pinned", [True, False], ids=["pinned", "pageable"])
 @pytest.mark.parametrize("path", [0, 1], ids=["auto", "general"])
 @pytest.mark.parametrize("last", ["shapelets", "gaussians", "points"])
-def test_simulate_host_overlapped_copy_back_is_bit_identical(ctx, torch_mod, last, path):
+def test_simulate_host_overlapped_copy_back_is_bit_identical(ctx, torch_mod, last, path, pinned):
     # woden_simulate_host hides the copy-back behind its LAST predictor (Gaussians, else points, else shapelets):
-    # on the channel-walking path tile by tile (12 channel tiles here, strided 2-D copies), on the general path
-    # and for a shapelet-only sky in chunks of time steps of >= 64 MB of output (7 steps of config 5's grid are
-    # 175 MB -> 3 ragged chunks of 2, 2, 3 steps).  Either way the result must equal the device path (the three
-    # calls in the same order) bit for bit, and the oracle on a sampled subset.
+    # on the channel-walking path, into a page-locked buffer, tile by tile (12 channel tiles here, strided 2-D
+    # copies); on the general path, for a shapelet-only sky and into pageable memory in chunks of time steps of
+    # >= 64 MB of output (7 steps of config 5's grid are 175 MB -> 3 ragged chunks of 2, 2, 3 steps).  Either way the
+    # result must equal the device path (the three calls in the same order) bit for bit, and the oracle on a
+    # sampled subset.
     import dataclasses
     wl = inputs.make_config(5, n_times=7, n_times_total=7)
     keep = lambda c, n: type(c)(**{f.name: (None if getattr(c, f.name) is None else getattr(c, f.name)[:n])
@@ -426,7 +439,7 @@ def test_simulate_host_overlapped_copy_back_is_bit_identical(ctx, torch_mod, las
     wl.points = keep(wl.points, 300) if last != "shapelets" else inputs.empty_components()
     wl.gaussians = keep(wl.gaussians, 200) if last == "gaussians" else inputs.empty_components()
     ctx.set_path(path)
-    out = np.full((wl.n_times, wl.n_freqs, wl.n_baselines), np.nan, dtype=np.complex64)
+    out, _keep = _host_vis(torch_mod, wl, pinned)
     assert out.nbytes > 2 * (64 << 20)
     ctx.simulate_host(wl, out)
     dev = _gpu_total(ctx, wl, path)
@@ -438,14 +451,15 @@ def test_simulate_host_overlapped_copy_back_is_bit_identical(ctx, torch_mod, las
     _assert_parity(out.reshape(-1)[idx], ref, scale, idx, wl, "simulate_host")
 
 
-def test_simulate_host_ragged_last_channel_tile(ctx, torch_mod):
-    # tile-wise copy-back with a ragged last tile (F = 75: tiles of 32, 32, 11 channels) and a pageable host buffer
+@pytest.mark.parametrize("pinned", [True, False], ids=["pinned", "pageable"])
+def test_simulate_host_ragged_last_channel_tile(ctx, torch_mod, pinned):
+    # tile-wise copy-back (page-locked buffer) with a ragged last tile: F = 75 -> tiles of 32, 32, 11 channels
     u, v, w, fr = _small_case(seed=5, T=3, B=300, F=75, uniform=True)
     wl = inputs.make_config(1)
     wl.u_m, wl.v_m, wl.w_m, wl.freqs_hz = u, v, w, fr
     wl.shapelets = inputs.empty_components()
     ctx.set_path(0)
-    out = np.full((wl.n_times, wl.n_freqs, wl.n_baselines), np.nan, dtype=np.complex64)
+    out, _keep = _host_vis(torch_mod, wl, pinned)
     ctx.simulate_host(wl, out)
     dev = _gpu_total(ctx, wl, 0)
     assert np.array_equal(out, dev)
