@@ -56,6 +56,7 @@ extern "C" {
 #define WODEN_ERR_CUDA          -4   /* CUDA allocation / launch / copy failed (woden_last_error) */
 #define WODEN_ERR_UNIMPLEMENTED -5
 #define WODEN_ERR_DATA          -6   /* woden_check(): a device-side precondition was violated  */
+#define WODEN_ERR_STATIC_LIMIT  -7   /* woden_truncate_select_static(): n beyond the built-in scratch */
 
 #define WODEN_MAX_ORDER 100          /* largest shapelet order n1 + n2 (paper uses <= 86, :183) */
 
@@ -292,6 +293,30 @@ int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, doub
  * compared with f_comp * total * (1 + 1e-15).  0 <= n <= 2^20 (ranking is by counting, O(n^2)). */
 int woden_truncate_select(woden_ctx *ctx, int n, const double *weights, double f_comp, int *keep, int *n_keep,
                           void *cuda_stream);
+
+/* The same selection (Eq 23-24; same arguments, same results bit for bit) for callers
+ * that must not allocate device memory: a stage running inside a host framework's fixed device arena, a
+ * plug-in called while the allocator is locked, a process under a hard GPU memory quota, a real-time
+ * loop that cannot take the device-wide stall cudaMalloc / cudaFree may cause.  It needs no woden_ctx
+ * and calls no cudaMalloc, cudaFree or other allocating routine: the ranked list is kept in a fixed
+ * array inside the library image, WODEN_STATIC_TRUNCATE_MAX entries (192 KiB).  Every GPU that loads
+ * the library holds that array until the process exits, used or not.
+ *   - n > WODEN_STATIC_TRUNCATE_MAX returns WODEN_ERR_STATIC_LIMIT and does nothing (use
+ *     woden_truncate_select for longer lists); other argument errors as for woden_truncate_select.
+ *   - weights, keep, n_keep: DEVICE pointers on the CURRENT device, owned by the caller; the call is
+ *     asynchronous on cuda_stream.
+ *   - The first call on each device looks up that device's address of the array (cudaGetSymbolAddress,
+ *     with that device current).  Make that first call outside any stream capture.
+ *   - All calls on a device share the one array, which keeps the last call's contents (each call clears
+ *     the part it uses first).  Two calls that overlap on the GPU -- different streams with no ordering
+ *     between them, or two host threads -- race on it and return garbage: keep calls on one stream or
+ *     order them with events.
+ * woden_static_last_error(): text of this thread's last failure in woden_truncate_select_static ("" if
+ * the last call succeeded); pointer owned by the library. */
+#define WODEN_STATIC_TRUNCATE_MAX 16384
+int woden_truncate_select_static(int n, const double *weights, double f_comp, int *keep, int *n_keep,
+                                 void *cuda_stream);
+const char *woden_static_last_error(void);
 
 /* Measurement aid: device time in milliseconds of the Gram-matrix kernel (the tcgen05 contraction) of
  * the LAST (beta1, beta2) pair of the last woden_fit_shapelets call on this context, from CUDA events

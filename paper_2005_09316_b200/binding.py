@@ -23,7 +23,9 @@ WODEN_ERR_ORDER = -3
 WODEN_ERR_CUDA = -4
 WODEN_ERR_UNIMPLEMENTED = -5
 WODEN_ERR_DATA = -6
+WODEN_ERR_STATIC_LIMIT = -7
 WODEN_MAX_ORDER = 100
+WODEN_STATIC_TRUNCATE_MAX = 16384
 WODEN_PATH_AUTO = 0
 WODEN_PATH_GENERAL = 1
 WODEN_PATH_NONE = -1
@@ -41,7 +43,7 @@ EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error"
            "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
            "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms", "woden_shapelet_basis_sums",
-           "woden_truncate_select"]
+           "woden_truncate_select", "woden_truncate_select_static", "woden_static_last_error"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -120,6 +122,9 @@ def load() -> C.CDLL:
     L.woden_shapelet_basis_sums.argtypes = [_vp, C.POINTER(woden_image_grid), C.c_double, C.c_double, C.c_double, C.c_int,
                                             C.c_double, C.c_double, C.POINTER(woden_restoring_beam), _vp, _vp]
     L.woden_truncate_select.argtypes = [_vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp]
+    L.woden_truncate_select_static.argtypes = [C.c_int, _vp, C.c_double, _vp, _vp, _vp]
+    L.woden_static_last_error.restype = C.c_char_p
+    L.woden_static_last_error.argtypes = []
     L.woden_fit_shapelets.argtypes = [_vp, C.POINTER(woden_image_grid), _vp, C.c_double, C.c_double, C.c_double, C.c_int,
                                       C.c_int, _dp, _dp, C.POINTER(woden_restoring_beam), C.c_int, _vp, _vp, _vp, _vp, _vp]
     L.woden_uvw_from_antennas.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_int, _dp, C.c_double, _vp, _vp, _vp, _vp]
@@ -130,7 +135,7 @@ def load() -> C.CDLL:
         if name == "woden_kernel_launches":
             L.woden_kernel_launches.restype = C.c_ulonglong
             L.woden_kernel_launches.argtypes = []
-        elif name not in ("woden_strerror", "woden_last_error"):
+        elif name not in ("woden_strerror", "woden_last_error", "woden_static_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -411,6 +416,26 @@ class Woden:
         rc = self._L.woden_pipe_rate(self._ctx, PIPES[which], int(iters), C.byref(ops), C.byref(clk))
         self._ck(rc, "woden_pipe_rate")
         return ops.value, clk.value
+
+
+def truncate_select_static(weights, f_comp: float, keep, n_keep, stream=None) -> None:
+    """woden_truncate_select_static: Eq 23-24 for callers that may not allocate device memory (code
+    running inside a framework's fixed device arena, under a memory quota, or in a loop that cannot
+    afford cudaMalloc's device-wide stall).  Nothing is allocated here either: `weights` (float64 [n]),
+    `keep` (int32 [n]) and `n_keep` (int32 [1]) are the caller's own tensors on the current device, and no
+    context is needed.  n above WODEN_STATIC_TRUNCATE_MAX raises WodenError(WODEN_ERR_STATIC_LIMIT).
+    Calls share one built-in scratch array per GPU: do not let two of them overlap on the device."""
+    import torch
+    if weights.dtype != torch.float64 or weights.dim() != 1:
+        raise ValueError("weights must be a 1-D float64 device tensor")
+    n = int(weights.numel())
+    if keep.dtype != torch.int32 or n_keep.dtype != torch.int32 or keep.numel() < n or n_keep.numel() < 1:
+        raise ValueError("keep must be int32 [n] and n_keep int32 [1]")
+    L = load()
+    rc = L.woden_truncate_select_static(n, _ptr(weights) if n else None, float(f_comp), _ptr(keep) if n else None,
+                                        _ptr(n_keep), _stream_handle(stream))
+    if rc != WODEN_OK:
+        raise WodenError(rc, "woden_truncate_select_static: " + L.woden_static_last_error().decode())
 
 
 def kernel_launches() -> int:

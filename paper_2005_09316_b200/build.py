@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libwoden_b200.so")
-SOURCES = ["api.cu", "pack.cu", "predict_pg.cu", "predict_walk.cu", "predict_shapelets.cu", "predict_shapelets_mma.cu", "geometry.cu", "calibrate.cu", "basis_lut.cu", "fit.cu", "truncate.cu", "pipes.cu"]
+SOURCES = ["api.cu", "pack.cu", "predict_pg.cu", "predict_walk.cu", "predict_shapelets.cu", "predict_shapelets_mma.cu", "geometry.cu", "calibrate.cu", "basis_lut.cu", "fit.cu", "truncate.cu", "truncate_static.cu", "pipes.cu"]
 HEADERS = ["kernels.h", "layout.h", "ptx.cuh", "phase.cuh", "hermite_rec.cuh", os.path.join("..", "..", "include", "woden_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

@@ -260,6 +260,7 @@ const char *woden_strerror(int status)
     case WODEN_ERR_CUDA: return "CUDA error (see woden_last_error)";
     case WODEN_ERR_UNIMPLEMENTED: return "not implemented";
     case WODEN_ERR_DATA: return "device-side precondition violated (see woden_b200.h)";
+    case WODEN_ERR_STATIC_LIMIT: return "size beyond the built-in scratch array of a non-allocating entry point";
     }
     return "unknown status";
 }

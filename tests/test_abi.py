@@ -43,7 +43,7 @@ def test_status_strings_and_constants_match_header():
         else:
             assert getattr(binding, name) == int(val), name
     assert pipes == binding.PIPES          # every pattern bench.py uses is a documented id
-    for code in (0, -1, -2, -3, -4, -5, -6):
+    for code in (0, -1, -2, -3, -4, -5, -6, -7):
         assert L.woden_strerror(code).decode() not in ("", "unknown status")
     assert L.woden_strerror(-99).decode() == "unknown status"
 
