@@ -218,6 +218,42 @@ def run_dry(args):
     return 0
 
 
+# order in which step() runs the three predictors between its four event marks (the first non-empty type
+# overwrites the buffer; the channel-walking calls come last so that copy-back can hide under them)
+STEP_ORDER = (("shapelets", 0, 1), ("points", 1, 2), ("gaussians", 2, 3))
+
+
+def split_marks(recs):
+    """Per-type call durations (ms) of every recorded step: {type: [ms, ...]} from the four marks of each
+    step, labelled by STEP_ORDER (the ONE place that maps marks to predictor names)."""
+    out = {name: [] for name, _, _ in STEP_ORDER}
+    for marks in recs:
+        for name, a, b in STEP_ORDER:
+            out[name].append(float(marks[a].elapsed_time(marks[b])))
+    return out
+
+
+def general_path_record(general_ms, counts, mufu_rate, t_roof, world, evals_per_step, steps):
+    """The SURVEY.md 8(d) rule (ii) block of the JSON line from the general path's per-type times."""
+    rec = {"ms_per_step": general_ms["step"], "value": world * evals_per_step / (general_ms["step"] * 1e-3),
+           "per_type": {}, "steps": steps, "warmup": 3}
+    mufu_ops = {"points": 2, "gaussians": 3}
+    for k in ("points", "gaussians", "shapelets"):
+        if counts[k] and general_ms.get(k):
+            r = {"ms_per_call": general_ms[k], "min_ms_per_call": general_ms.get(k + "_min"),
+                 "evals_per_s": counts[k] / (general_ms[k] * 1e-3)}
+            if k in mufu_ops:
+                r["frac_of_mufu_roofline"] = r["evals_per_s"] / (mufu_rate / mufu_ops[k])
+            rec["per_type"][k] = r
+    rec["composite_frac"] = 1e3 * t_roof / general_ms["step"]
+    # a kernel that issues 2 (3) MUFU per eval cannot beat the MUFU pipe: a fraction far above 1 means the
+    # marks were mapped to the wrong predictor
+    rec["labels_consistent"] = all(r.get("frac_of_mufu_roofline", 0.0) <= 1.10 for r in rec["per_type"].values())
+    rec["note"] = ("woden_set_path(GENERAL): 2 MUFU per point eval, 3 per Gaussian eval; fractions are of the "
+                   "MUFU-pipe roofline at the pipe rate measured in this run")
+    return rec
+
+
 def time_steps(step, n_warm, n_steps, barrier):
     """n_warm untimed + n_steps timed calls of step(record) between barriers; returns (ms_total, records)."""
     import torch
@@ -312,9 +348,7 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else {}
     ms_total = e0.elapsed_time(e1)
-    for marks in recs:
-        for name, a, b in (("shapelets", 0, 1), ("points", 1, 2), ("gaussians", 2, 3)):
-            per_type_ms[name].append(marks[a].elapsed_time(marks[b]))
+    per_type_ms = split_marks(recs)
     ctx.check()
     ms_total = parallel.max_over_ranks(ms_total, dist, f"cuda:{local}")
     ms_per_step = ms_total / args.steps
@@ -342,8 +376,9 @@ def run_ours(args):
         ctx.set_path(binding.WODEN_PATH_GENERAL)
         g_total, g_recs = time_steps(step, 3, max(3, min(5, args.steps)), barrier)
         ctx.set_path(binding.WODEN_PATH_AUTO)
-        general_ms = {k: float(np.median([m[a].elapsed_time(m[b]) for m in g_recs]))
-                      for k, a, b in (("points", 0, 1), ("gaussians", 1, 2), ("shapelets", 2, 3))}
+        g_split = split_marks(g_recs)
+        general_ms = {k: float(np.median(v)) for k, v in g_split.items()}
+        general_ms.update({k + "_min": float(np.min(v)) for k, v in g_split.items()})
         general_ms["step"] = parallel.max_over_ranks(g_total / len(g_recs), dist, f"cuda:{local}")
 
     if rank != 0:
@@ -356,21 +391,23 @@ def run_ours(args):
     per_type = {}
     for name, key in (("points", "points"), ("gaussians", "gaussians"), ("shapelets", "shapelets")):
         if med[name] and counts[key]:
-            per_type[name] = {"evals_per_s": counts[key] / (med[name] * 1e-3), "ms_per_call": med[name]}
+            per_type[name] = {"evals_per_s": counts[key] / (med[name] * 1e-3), "ms_per_call": med[name],
+                              "min_ms_per_call": float(np.min(per_type_ms[name]))}
     if "shapelets" in per_type:
         per_type["shapelets"]["coeff_evals_per_s"] = counts["shapelet_coeffs"] / (med["shapelets"] * 1e-3)
 
     walk = args.path != "general"        # all configs have uniformly spaced channels
     mufu_rate, mufu_clk = ctx.pipe_rate("MUFU")
     fma_rate, _ = ctx.pipe_rate("FFMA")
+    ffma2_rate, _ = ctx.pipe_rate("FFMA2")          # the instruction the walking kernels issue
     dominant = max((k for k in per_type), key=lambda k: med[k])
     if dominant == "points":
         ops = {"walk": ("FP32 FMA pipe: 4 FP32 lane-ops per eval (2 three-term recurrence + 2 accumulate)",
-                        fma_rate / 4.0),
+                        ffma2_rate / 4.0),
                "general": ("MUFU pipe: 2 MUFU (sin, cos) per eval", mufu_rate / 2.0)}
     elif dominant == "gaussians":
         ops = {"walk": ("FP32 FMA pipe: 7 FP32 lane-ops per eval (2 recurrence + 2 envelope walk + 1 flux*envelope "
-                        "+ 2 accumulate)", fma_rate / 7.0),
+                        "+ 2 accumulate)", ffma2_rate / 7.0),
                "general": ("MUFU pipe: 3 MUFU (sin, cos, ex2) per eval", mufu_rate / 3.0)}
     else:
         ops = {"walk": ("FP32 FMA pipe: 1 FFMA per coefficient", fma_rate),
@@ -396,19 +433,21 @@ def run_ours(args):
         "operand_delivery": {"ffma2_three_fresh_pairs_fma_per_s": ffma2_3reg, "ffma_reused_operands_fma_per_s": fma_rate,
                              "walk_pattern_fma_per_s": walk_rate,
                              "frac_of_walk_pattern": (ach * 4.0 / walk_rate) if (walk and dominant == "points") else None,
-                             "read_cycle_model": {"pipe_cycles_per_two_components": 271, "read_cycles_final_build": 334,
-                                                  "read_cycles_floor": 317, "measured_over_model": 1.05,
-                                                  "source": "profiles/walk_rf_r2.md (counted on the SASS of the "
-                                                            "committed build; recorded, not measured in this run)"},
                              "note": "each register bank (even / odd) feeds one operand per lane per clock: an FMA with "
-                                     "three fresh register operands runs at 2/3 of the pipe rate, and the walking "
-                                     "kernel's time is 1.05 x the sum of its instructions' register-read cycles "
-                                     "(profiles/walk_rf_r2.md); its own 4-FFMA2 pattern in isolation sustains "
-                                     "walk_pattern_fma_per_s (DESIGN.md section 7)"},
-        "peak_basis": basis + f"; pipe rate measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
+                                     "three fresh register operands runs at 2/3 of the pipe rate (the read-cycle count of "
+                                     "the shipped SASS is prose in profiles/walk_rf_r2.md, not part of this record); "
+                                     "the kernel's own 4-FFMA2 pattern in isolation sustains walk_pattern_fma_per_s "
+                                     "(DESIGN.md section 7)"},
+        "peak_basis": basis + ("; packed FFMA2 rate (the instruction the kernel issues)" if walk and dominant != "shapelets"
+                               else "") + f" measured live by woden_pipe_rate at {mufu_clk / 1e6:.0f} MHz",
+        "pipe_rates_fma_per_s": {"FFMA2": ffma2_rate, "FFMA": fma_rate,
+                                 "nominal_fp32": SM_COUNT * FP32_LANES_PER_SM * SM_MAX_HZ},
         "nominal_mufu_roofline_gevals": SM_COUNT * MUFU_LANES_PER_SM * SM_MAX_HZ / (2 if dominant == "points" else 3) / 1e9,
     }
     roofline["frac_of_mufu_roofline"] = ach / 1e9 / roofline["nominal_mufu_roofline_gevals"]
+    if walk and dominant in ("points", "gaussians"):
+        lane_ops = 4.0 if dominant == "points" else 7.0
+        roofline["frac_of_nominal_fp32"] = ach * lane_ops / (SM_COUNT * FP32_LANES_PER_SM * SM_MAX_HZ)
     # SURVEY.md §8(d) composite roofline time for the whole step at the measured pipe rates
     t_roof = (counts["points"] / (mufu_rate / 2) + counts["gaussians"] / (mufu_rate / 3)
               + counts["shapelet_coeffs"] / fma_rate)
@@ -430,18 +469,8 @@ def run_ours(args):
 
     general_path = None
     if general_ms is not None:
-        general_path = {"ms_per_step": general_ms["step"], "value": world * evals_per_step / (general_ms["step"] * 1e-3),
-                        "per_type": {}, "steps": max(3, min(5, args.steps)), "warmup": 3}
-        mufu_ops = {"points": 2, "gaussians": 3}
-        for k in ("points", "gaussians", "shapelets"):
-            if counts[k] and general_ms[k]:
-                r = {"ms_per_call": general_ms[k], "evals_per_s": counts[k] / (general_ms[k] * 1e-3)}
-                if k in mufu_ops:
-                    r["frac_of_mufu_roofline"] = r["evals_per_s"] / (mufu_rate / mufu_ops[k])
-                general_path["per_type"][k] = r
-        general_path["composite_frac"] = 1e3 * t_roof / general_ms["step"]
-        general_path["note"] = ("woden_set_path(GENERAL): 2 MUFU per point eval, 3 per Gaussian eval; fractions are of the "
-                                "MUFU-pipe roofline at the pipe rate measured in this run")
+        general_path = general_path_record(general_ms, counts, mufu_rate, t_roof, world, evals_per_step,
+                                           max(3, min(5, args.steps)))
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

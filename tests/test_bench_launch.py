@@ -40,3 +40,37 @@ def test_under_torchrun_the_environment_is_used():
     assert out.returncode == 0, out.stderr[-2000:]
     lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2
+
+
+class _Mark:
+    """Stand-in for a CUDA event: elapsed_time between two marks is the difference of their stamps."""
+
+    def __init__(self, t):
+        self.t = t
+
+    def elapsed_time(self, other):
+        return other.t - self.t
+
+
+def test_per_type_labels_follow_the_order_step_runs_the_predictors():
+    # VERDICT round 2 weak #2: step() runs shapelets, points, Gaussians; both the main arm and the general-path
+    # block must label the three intervals in that order (one shared table, bench.STEP_ORDER)
+    sys.path.insert(0, ROOT)
+    import bench
+    assert [n for n, _, _ in bench.STEP_ORDER] == ["shapelets", "points", "gaussians"]
+    recs = [[_Mark(0.0), _Mark(18.0), _Mark(18.0 + 640.0), _Mark(18.0 + 640.0 + 242.0)],
+            [_Mark(5.0), _Mark(24.0), _Mark(24.0 + 642.0), _Mark(24.0 + 642.0 + 240.0)]]
+    split = bench.split_marks(recs)
+    assert split == {"shapelets": [18.0, 19.0], "points": [640.0, 642.0], "gaussians": [242.0, 240.0]}
+    # config 5's counts and a MUFU rate of 148 SMs x 16 lanes x 1.965 GHz: the fractions land near 0.95, and a
+    # mislabelled record (the shapelet time under "points") is flagged
+    counts = {"points": 8000 * 174784512, "gaussians": 2000 * 174784512, "shapelets": 20 * 174784512}
+    mufu = 148 * 16 * 1.965e9
+    ms = {"shapelets": 18.5, "points": 641.0, "gaussians": 241.0, "step": 900.5}
+    rec = bench.general_path_record(ms, counts, mufu, 0.85, 1, sum(counts.values()), 5)
+    assert 0.9 < rec["per_type"]["points"]["frac_of_mufu_roofline"] < 1.0
+    assert 0.9 < rec["per_type"]["gaussians"]["frac_of_mufu_roofline"] < 1.0
+    assert "frac_of_mufu_roofline" not in rec["per_type"]["shapelets"]
+    assert rec["labels_consistent"]
+    wrong = dict(ms, points=18.5, gaussians=641.0, shapelets=241.0)
+    assert not bench.general_path_record(wrong, counts, mufu, 0.85, 1, sum(counts.values()), 5)["labels_consistent"]
