@@ -554,8 +554,16 @@ def run_truncation(args):
             ctx.predict_shapelets(uvw, *ds_[:4], wl.ref_freq_hz, *ds_[4:], di[0], int(s.coeff.size), pmax,
                                   di[1], di[2], dc, vis, False)
 
-        rows.append({"f_comp": f, "msclean_components": p.n + g.n, "msclean_ms": timed(clean),
-                     "shapelet_basis_functions": int(s.coeff.size), "shapelet_p_max": pmax, "shapelet_ms": timed(shp)})
+        row = {"f_comp": f, "msclean_components": p.n + g.n, "msclean_ms": timed(clean),
+               "shapelet_basis_functions": int(s.coeff.size), "shapelet_p_max": pmax, "shapelet_ms": timed(shp)}
+        eng, bucket = ctx.last_shapelet_path()
+        row["shapelet_engine_auto"] = {1: "register", 2: "tensor", 3: "register-sparse"}.get(eng, str(eng))
+        row["shapelet_order_bucket"] = bucket
+        for name, code in (("register", 1), ("tensor", 2)):          # the two engines forced, for AUTO's policy table
+            ctx.set_shapelet_path(code)
+            row[f"shapelet_ms_{name}"] = timed(shp)
+        ctx.set_shapelet_path(0)
+        rows.append(row)
     ctx.check()
     print(json.dumps({"truncation": rows, "workload": "config 4 (8128 baselines x 14 steps x 384 channels)",
                       "note": "one launch set per model; medians of CUDA-event times"}))

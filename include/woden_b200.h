@@ -108,6 +108,15 @@ int woden_last_path(const woden_ctx *ctx);
 #define WODEN_SHAPELET_REGISTER 1
 #define WODEN_SHAPELET_TENSOR   2
 int woden_set_shapelet_path(woden_ctx *ctx, int path);
+/* Which shapelet engine the last woden_predict_shapelets call on this context launched, and at which
+ * compile-time order bucket (the kernels are instantiated for orders 4, 8, 12, 16, 20, 24, 32, 40, 48, 60, 72,
+ * 86, 100; a call runs the smallest bucket >= p_max): WODEN_SHAPELET_REGISTER, WODEN_SHAPELET_REGISTER_SPARSE
+ * (the register engine's variant that skips empty 4-coefficient chunks of truncated models,
+ * PAPER.md:271-284), WODEN_SHAPELET_TENSOR, or WODEN_PATH_NONE (n == 0 / no call yet; bucket -1).
+ * For tests and reports; never changes behaviour. */
+#define WODEN_SHAPELET_REGISTER_SPARSE 3
+int woden_last_shapelet_path(const woden_ctx *ctx);
+int woden_last_shapelet_bucket(const woden_ctx *ctx);
 
 /* Baseline coordinates and channels ("array layout and observation parameters"). */
 typedef struct {

@@ -33,6 +33,7 @@ WODEN_PATH_WALKING = 2
 WODEN_SHAPELET_AUTO = 0
 WODEN_SHAPELET_REGISTER = 1
 WODEN_SHAPELET_TENSOR = 2
+WODEN_SHAPELET_REGISTER_SPARSE = 3
 WODEN_BASIS_RECURRENCE = 0
 WODEN_BASIS_LUT = 1
 WODEN_FIT_MAX_ORDER = 86
@@ -40,7 +41,7 @@ PIPES = {"FFMA": 0, "MUFU": 1, "DFMA": 2, "I2F": 3, "LOP3": 4, "FFMA2": 5, "FFMA
          "MUFU_EX2": 8, "MUFU_FFMA": 9, "FFMA_3REG": 10, "FFMA2_3REG": 11, "FFMA2_BCAST": 12, "FFMA2_UR": 13, "WALK": 14}
 
 EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error", "woden_check",
-           "woden_set_path", "woden_last_path", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
+           "woden_set_path", "woden_last_path", "woden_last_shapelet_path", "woden_last_shapelet_bucket", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
            "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms", "woden_shapelet_basis_sums",
            "woden_truncate_select", "woden_truncate_select_static", "woden_static_last_error"]
@@ -107,6 +108,8 @@ def load() -> C.CDLL:
     L.woden_check.argtypes = [_vp]
     L.woden_set_path.argtypes = [_vp, C.c_int]
     L.woden_last_path.argtypes = [_vp]
+    L.woden_last_shapelet_path.argtypes = [_vp]
+    L.woden_last_shapelet_bucket.argtypes = [_vp]
     L.woden_set_shapelet_path.argtypes = [_vp, C.c_int]
     L.woden_shapelet_series.argtypes = [_vp, C.c_int, C.c_int, C.c_longlong, _vp, _vp, C.c_double, C.c_double, _vp, _vp]
     common = [_vp, C.POINTER(woden_uvw), C.c_int, _vp, _vp, _vp, _vp, C.c_double]
@@ -222,6 +225,11 @@ class Woden:
 
     def last_path(self) -> int:
         return int(self._L.woden_last_path(self._ctx))
+
+    def last_shapelet_path(self):
+        """(engine, order bucket) of the last predict_shapelets call: WODEN_SHAPELET_REGISTER / _REGISTER_SPARSE /
+        _TENSOR (WODEN_PATH_NONE, -1 when nothing was launched)."""
+        return (int(self._L.woden_last_shapelet_path(self._ctx)), int(self._L.woden_last_shapelet_bucket(self._ctx)))
 
     def set_shapelet_path(self, path: int):
         self._ck(self._L.woden_set_shapelet_path(self._ctx, int(path)), "woden_set_shapelet_path")

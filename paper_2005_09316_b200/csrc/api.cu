@@ -46,6 +46,7 @@ struct woden_ctx {
     int lut_pm = -1, lut_nx = 0;
     double lut_dx = 0.0;
     int shapelet_path = WODEN_SHAPELET_AUTO;
+    int last_shapelet_path = WODEN_PATH_NONE, last_shapelet_bucket = -1;
     std::vector<double> chan_freqs;      // frequencies the device channel table was built from
     std::vector<double> chan_s_host;     // nu_f / c of the padded channel list (host copy)
     cudaStream_t walk_stream = nullptr;  // second lane of the channel-walking launches
@@ -279,6 +280,9 @@ unsigned long long woden_kernel_launches(void) { return woden::g_kernel_launches
 
 int woden_last_path(const woden_ctx *ctx) { return ctx ? ctx->last_path : WODEN_PATH_NONE; }
 
+int woden_last_shapelet_path(const woden_ctx *ctx) { return ctx ? ctx->last_shapelet_path : WODEN_PATH_NONE; }
+int woden_last_shapelet_bucket(const woden_ctx *ctx) { return ctx ? ctx->last_shapelet_bucket : -1; }
+
 int woden_set_shapelet_path(woden_ctx *ctx, int path)
 {
     if (!ctx) return WODEN_ERR_NULL;
@@ -406,6 +410,8 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ctx->last_stream = st;
+    ctx->last_shapelet_path = WODEN_PATH_NONE;
+    ctx->last_shapelet_bucket = -1;
     if (n == 0) return zero_or_nothing(ctx, uvw, vis, accumulate, st);
     if ((rc = ensure_err(ctx, st)) != WODEN_OK) return rc;
     if ((rc = ensure_chan(ctx, uvw, st)) != WODEN_OK) return rc;
@@ -430,6 +436,8 @@ int woden_predict_shapelets(woden_ctx *ctx, const woden_uvw *uvw, int n, const d
     // AUTO takes it from the order bucket at which it measured faster (profiles/shapelet_mma_r2.md)
     const bool tensor = ctx->shapelet_path == WODEN_SHAPELET_TENSOR ||
                         (ctx->shapelet_path == WODEN_SHAPELET_AUTO && PM >= SHAPELET_TENSOR_MIN_ORDER);
+    ctx->last_shapelet_bucket = PM;
+    ctx->last_shapelet_path = tensor ? WODEN_SHAPELET_TENSOR : sparse ? WODEN_SHAPELET_REGISTER_SPARSE : WODEN_SHAPELET_REGISTER;
     if (tensor) {
         CU(ctx, ctx->bmat.reserve(mma_bmat_halves(PM, n) * 2), "alloc coefficient matrices");
         CU(ctx, ctx->bscale.reserve((size_t)n * 4), "alloc coefficient scales");

@@ -199,11 +199,34 @@ def _run_shapelets(ctx, torch, u, v, w, fr, l, m, s0, al, b1, b2, pa, M, off, n1
     return vis.cpu().numpy()
 
 
-@pytest.mark.parametrize("engine", [1, 2], ids=["register", "tensor"])
-@pytest.mark.parametrize("p_max", [0, 1, 5, 13, 40, 61, 86, 100])
+ORDER_BUCKETS = (4, 8, 12, 16, 20, 24, 32, 40, 48, 60, 72, 86, 100)     # the kernels' compile-time orders
+TENSOR_FROM = 24                                                          # AUTO's switch (api.cu)
+# every bucket edge and the order just above it (which must take the next bucket), plus 0 and 1
+BUCKET_EDGE_ORDERS = [0, 1] + sorted(set(ORDER_BUCKETS) | {b + 1 for b in ORDER_BUCKETS[:-1]})
+
+
+def _bucket_of(p_max):
+    return next(b for b in ORDER_BUCKETS if p_max <= b)
+
+
+def _is_sparse(n_coeff, n, bucket):
+    return n_coeff < 0.75 * n * ((bucket + 1) * (bucket + 2) // 2)      # api.cu: chunk-skipping variant below 3/4
+
+
+def _expected_engine(engine, bucket, sparse):
+    from paper_2005_09316_b200 import binding
+    if engine == 2 or (engine == 0 and bucket >= TENSOR_FROM):
+        return binding.WODEN_SHAPELET_TENSOR
+    return binding.WODEN_SHAPELET_REGISTER_SPARSE if sparse else binding.WODEN_SHAPELET_REGISTER
+
+
+@pytest.mark.parametrize("engine", [1, 2, 0], ids=["register", "tensor", "auto"])
+@pytest.mark.parametrize("p_max", BUCKET_EDGE_ORDERS)
 def test_shapelets_orders_up_to_the_limit(ctx, torch_mod, p_max, engine):
-    # full triangles at every bucket edge incl. the paper's p_max = 86 and the
-    # library limit; beta up to 20 arcmin on a 3 km array reaches Hermite arguments ~30 (H4)
+    # full triangles at EVERY order bucket's edge and the order above it, on both engines and under AUTO
+    # (each bucket is its own template instantiation with its own tiling and descriptor table), incl. the
+    # paper's p_max = 86 and the library limit; beta up to 20 arcmin on a 3 km array reaches
+    # Hermite arguments ~30 (H4).  Eq 15-17.
     ctx.set_path(0)
     ctx.set_shapelet_path(engine)
     u, v, w, fr = _small_case(seed=p_max, T=2, B=333, F=5)
@@ -221,11 +244,84 @@ def test_shapelets_orders_up_to_the_limit(ctx, torch_mod, p_max, engine):
     cf = rng.normal(0, 1, n * P) * np.exp(-(n1 + n2) / 10.0)
     off = np.arange(n + 1) * P
     V = _run_shapelets(ctx, torch_mod, u, v, w, fr, l, m, s0, al, b1, b2, pa, M, off, n1, n2, cf, p_max)
+    ran = ctx.last_shapelet_path()
     ref = oracle.predict_shapelets(u, v, w, fr, l, m, s0, al, 150e6, b1, b2, pa, M, off, n1, n2, cf)
     scale = oracle.tolerance_scale(fr, s0, al, 150e6, off, cf)
     ctx.set_shapelet_path(0)
+    bucket = _bucket_of(p_max)
+    sparse = _is_sparse(n * P, n, bucket)
+    assert ran == (_expected_engine(engine, bucket, sparse), bucket)
     err = np.abs(V - ref) / scale[None, :, None]
     assert err.max() <= TOL
+    assert np.abs(ref).max() > 1e-3
+
+
+@pytest.mark.parametrize("engine", [0, 2, 1], ids=["auto", "tensor", "register"])
+@pytest.mark.parametrize("f_keep", [0.6, 0.2])
+@pytest.mark.parametrize("p_max", [b for b in ORDER_BUCKETS if b >= TENSOR_FROM] + [23, 29, 42])
+def test_truncated_triangles_on_every_tensor_bucket(ctx, torch_mod, p_max, f_keep, engine):
+    # PAPER.md:267-288 (Eq 23-25): a model truncated to a fraction of its ranked absolute weight is a SPARSE
+    # coefficient list whose highest surviving order decides the bucket.  Every bucket AUTO gives to the tensor
+    # engine (and the p_max = 42 / 29 / 23 of config 4's truncated models, profiles/truncation_r2.md) is run
+    # under AUTO, forced TENSOR and forced REGISTER against the oracle on the same ragged, unsorted lists.
+    from oracle import truncate as otrunc
+    ctx.set_path(0)
+    ctx.set_shapelet_path(engine)
+    u, v, w, fr = _small_case(seed=500 + p_max, T=2, B=257, F=3)
+    rng = np.random.default_rng(7000 + 10 * p_max + int(10 * f_keep))
+    n = 2
+    l, m = inputs.disk_lm(rng, n, 10.0)
+    s0 = np.array([1.3, 0.6]); al = np.array([-0.7, -1.0])
+    b1 = np.array([4.0, 9.0]) * inputs.ARCMIN; b2 = np.array([6.0, 3.0]) * inputs.ARCMIN
+    pa = rng.uniform(0, np.pi, n)
+    M = inputs.local_uv_basis(l, m)
+    t1, t2 = inputs.full_triangle(p_max)
+    n1l, n2l, cfl, off = [], [], [], [0]
+    for j in range(n):
+        cf = rng.normal(0, 1, len(t1)) * np.exp(-(t1 + t2) / 8.0)
+        keep = otrunc.keep_mask(cf, f_keep)                       # Eq 23-24 on |C| (Eq 25 with unit basis sums)
+        keep[np.flatnonzero(t1 + t2 == p_max)[j]] = True           # one term of the highest order survives
+        idx = rng.permutation(np.flatnonzero(keep))                # the list order is free
+        n1l.append(t1[idx]); n2l.append(t2[idx]); cfl.append(cf[idx]); off.append(off[-1] + idx.size)
+    n1, n2, cf = np.concatenate(n1l), np.concatenate(n2l), np.concatenate(cfl)
+    bucket = _bucket_of(p_max)
+    sparse = _is_sparse(cf.size, n, bucket)
+    assert sparse and cf.size < 0.5 * n * len(t1)
+    V = _run_shapelets(ctx, torch_mod, u, v, w, fr, l, m, s0, al, b1, b2, pa, M, off, n1, n2, cf, p_max)
+    ran = ctx.last_shapelet_path()
+    ctx.set_shapelet_path(0)
+    assert ran == (_expected_engine(engine, bucket, sparse), bucket)
+    ref = oracle.predict_shapelets(u, v, w, fr, l, m, s0, al, 150e6, b1, b2, pa, M, off, n1, n2, cf)
+    scale = oracle.tolerance_scale(fr, s0, al, 150e6, off, cf)
+    assert (np.abs(V - ref) / scale[None, :, None]).max() <= TOL
+    assert np.abs(ref).max() > 1e-3
+
+
+@pytest.mark.parametrize("engine", [0, 2, 1], ids=["auto", "tensor", "register"])
+@pytest.mark.parametrize("f_comp", [0.8, 0.6, 0.4, 0.2])
+def test_config4_models_truncated_by_eq25_weights_as_bench_times_them(ctx, torch_mod, f_comp, engine):
+    # the exact models `bench.py --truncation` times (config 4's two lobes ranked by Eq 25 with the restoring
+    # beam): p_max 42 / 29 / 23 / 17 -> buckets 48 / 32 / 24 / 20, here checked against the oracle
+    from paper_2005_09316_b200 import truncate
+    wl = inputs.make_config(4)
+    w_sh = truncate.shapelet_basis_weights(ctx, wl.shapelets)
+    s = truncate.truncate_shapelets(ctx, wl.shapelets, f_comp, w_sh)
+    ctx.set_path(0)
+    ctx.set_shapelet_path(engine)
+    u, v, w = (a[:2, :1200] for a in (wl.u_m, wl.v_m, wl.w_m))
+    fr = wl.freqs_hz[::64]
+    pmax = int((s.n1 + s.n2).max())
+    V = _run_shapelets(ctx, torch_mod, u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, s.beta1_rad, s.beta2_rad, s.pa_rad,
+                       s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff, pmax)
+    ran = ctx.last_shapelet_path()
+    ctx.set_shapelet_path(0)
+    bucket = _bucket_of(pmax)
+    sparse = _is_sparse(s.coeff.size, s.n, bucket)
+    assert ran == (_expected_engine(engine, bucket, sparse), bucket)
+    ref = oracle.predict_shapelets(u, v, w, fr, s.l, s.m, s.s0_jy, s.alpha, 150e6, s.beta1_rad, s.beta2_rad,
+                                   s.pa_rad, s.uv_basis, s.coeff_offset, s.n1, s.n2, s.coeff)
+    scale = oracle.tolerance_scale(fr, s.s0_jy, s.alpha, 150e6, s.coeff_offset, s.coeff)
+    assert (np.abs(V - ref) / scale[None, :, None]).max() <= TOL
     assert np.abs(ref).max() > 1e-3
 
 
