@@ -29,7 +29,11 @@
  * returns.  The library never frees or keeps caller pointers after the call's work has run.
  * Device calls only enqueue work on `cuda_stream` (a cudaStream_t, NULL = legacy default
  * stream) and return without synchronising; internal scratch belongs to the context, so one
- * context serves one stream at a time.
+ * context serves one stream at a time (a context's next call may go to another stream only after
+ * its previous call's work has finished).  Different contexts on one GPU are independent and may be
+ * driven from different host threads and streams: the one resource they share, the constant bank the
+ * channel-walking kernels read their component blocks from, is handed from call to call by the
+ * library (walking calls on one device run one after another on the GPU, whatever their streams).
  *
  * Output layout: complex64 interleaved (re, im), vis[((t * n_freqs) + f) * n_baselines + b].
  *

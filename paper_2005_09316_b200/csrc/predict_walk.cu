@@ -48,6 +48,7 @@
 // between the two halves of the bank and between two streams that own disjoint parts of the
 // output, so the copy into one half and the tail of one launch hide behind the launch running
 // from the other half.
+#include <mutex>
 #include <type_traits>
 
 #include "kernels.h"
@@ -318,6 +319,31 @@ __global__ void pack_walk_blocks_kernel(const Geo *__restrict__ geo, const doubl
     if (pos == 0) blk->rec[k % KC].geo = geo[k];
 }
 
+// Per-device ordering of the calls that refill CBANK (see launch()).
+constexpr int BANK_MAX_DEVICES = 64;
+std::mutex g_bank_mu[BANK_MAX_DEVICES];
+cudaEvent_t g_bank_done[BANK_MAX_DEVICES] = {};      // "the last walking call on this device has finished"
+
+struct BankOrder {
+    int dev = -1;
+    cudaError_t begin(cudaStream_t main)
+    {
+        int d = -1;
+        cudaError_t e = cudaGetDevice(&d);
+        if (e != cudaSuccess) return e;
+        if (d < 0 || d >= BANK_MAX_DEVICES) return cudaErrorInvalidDevice;
+        g_bank_mu[d].lock();
+        dev = d;
+        if (!g_bank_done[d]) {
+            e = cudaEventCreateWithFlags(&g_bank_done[d], cudaEventDisableTiming);
+            if (e != cudaSuccess) { g_bank_done[d] = nullptr; return e; }
+        }
+        return cudaStreamWaitEvent(main, g_bank_done[d], 0);      // the aux lane follows through the fork event
+    }
+    cudaError_t end(cudaStream_t main) { return dev >= 0 && g_bank_done[dev] ? cudaEventRecord(g_bank_done[dev], main) : cudaSuccess; }
+    ~BankOrder() { if (dev >= 0) g_bank_mu[dev].unlock(); }
+};
+
 template <bool GAUSS, typename Geo>
 cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *blocks, int n, float2 *vis,
                    int accumulate, unsigned int *err, const WalkStreams &ws)
@@ -329,9 +355,16 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *
     p.u_m = uvw.u_m; p.v_m = uvw.v_m; p.w_m = uvw.w_m; p.vis = vis;
     p.B = uvw.B; p.F = uvw.F; p.ds = ch.ds; p.err = err;
 
+    // CBANK is one symbol per device, shared by every context and stream of the process: walking calls on
+    // a device are ordered one after another.  The host lock keeps two threads' enqueue loops apart; the
+    // per-device event (recorded when a call's last launch has been enqueued, waited on by the next
+    // call's streams before its first bank copy) keeps their GPU work apart.  Successive calls on one
+    // stream wait on an event of their own stream: no cost on the usual path.
+    BankOrder order;
+    cudaError_t e = order.begin(ws.main);
     // Two lanes (bank half + stream each) that own disjoint outputs: whole channel tiles dealt
     // alternately, or the two halves of the (baseline, time) range when there is one tile.
-    cudaError_t e = cudaEventRecord(ws.fork, ws.main);
+    if (e == cudaSuccess) e = cudaEventRecord(ws.fork, ws.main);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(ws.aux, ws.fork, 0);
     const int n_units = n_ftiles >= 2 ? n_ftiles : 2;
     const long long half_bt = (n_bt / 2 + WTHREADS - 1) / WTHREADS * WTHREADS;
@@ -365,6 +398,7 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *
     // join even after an error so that the caller's stream stays ordered after the aux work
     cudaError_t e2 = cudaEventRecord(ws.join, ws.aux);
     if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(ws.main, ws.join, 0);
+    if (e2 == cudaSuccess) e2 = order.end(ws.main);
     return e != cudaSuccess ? e : e2;
 }
 
