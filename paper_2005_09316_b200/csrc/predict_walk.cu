@@ -4,26 +4,29 @@
 // (+1 for Gaussians) per component x visibility; this one spends 4 FP32 lane-operations.
 //
 // Mapping: one thread owns one (baseline, time) pair and WFT = 32 consecutive channels, held as
-// two chains of WH = 16 (channels j and j + 16) that ride in the two lanes of the packed FP32x2
-// instructions of sm_100 (SASS FFMA2 / FMUL2).  All 2 x 32 accumulators stay in registers for
+// ONE chain that is walked from its middle outwards: the two lanes of the packed FP32x2
+// instructions of sm_100 (SASS FFMA2 / FMUL2) carry the two DIRECTIONS (lane 0: channel J0+1+t,
+// lane 1: channel J0-t at step t = 0..15, J0 = 15).  All 2 x 32 accumulators stay in registers for
 // the sum over the components of one launch (no atomics; the paper's atomicAdd, is
 // prior art).
 //
 // Per (thread, component):
 //   D = u_m l + v_m m + w_m (n-1)                       FP64 metres (3 FP64 ops, hard part H1)
-//   seeds: q = exp(i theta) at chain position J0 = 7 of both chains by true sin/cos of the FP64
-//          phase reduced to its fraction as Q0.32 (4 MUFU), w = exp(i delta), delta = 2 pi D dnu/c (2 MUFU);
-//          position J0 + 1 by one complex rotation with w.
+//   seeds: q = exp(i theta) at chain position J0 = 15 by true sin/cos of the FP64 phase reduced to
+//          its fraction as Q0.32 (2 MUFU), w = exp(i delta), delta = 2 pi D dnu/c (2 MUFU);
+//          position J0 + 1 by one complex rotation with w.  ONE seed serves all 32 channels (the
+//          round-2 kernel seeded two chains of 16 with 6 MUFU).
 //   walk : with channels nu_0 + j dnu the real and imaginary parts of q_j each obey
 //          x_{j+1} = 2 cos(delta) x_j - x_{j-1}: ONE FMA per real number per channel.  The chain
-//          is walked from the middle outwards (7 steps each way), which bounds the growth of
-//          rounding error (~ steps^2 / 2 ulp); every new value is
-//          accumulated at once, so only two chain values per direction are live.
+//          is walked from the middle outwards (15 steps each way, both directions in one packed
+//          instruction), which bounds the growth of rounding error (~ steps^2 / 2 ulp, DESIGN.md
+//          "Tolerance"); every new value is accumulated at once, so only two chain values are live.
 //   PTX has no negate for f32x2, so the recurrence runs on y_j = s_j x_j with the sign pattern
 //   s = (+,+,-,-) repeating from J0: y_{j+1} = (s_{j+1} s_j) c y_j + y_{j-1} needs only the
-//   scalars +c / -c, and s_j is applied once per visibility in the epilogue.
-//   Gaussians: xi_j = exp2(-Q s_j^2), s_j = nu_j / c, is walked both ways by the second-order
-//   multiplicative recurrence xi_{j+1} = xi_j rho_j, rho_{j+1} = rho_j qq (7 MUFU seeds).
+//   scalars +c / -c, and s_j is applied once per visibility in the epilogue.  The pattern is
+//   symmetric about J0 + 1/2, so both lanes of a step carry the same sign: s(t) = - for t mod 4 in {1, 2}.
+//   Gaussians: xi_j = exp2(-Q s_j^2), s_j = nu_j / c, is walked both ways (one lane each) by the
+//   second-order multiplicative recurrence xi_{t+1} = xi_t rho_t, rho_{t+1} = rho_t qq (5 MUFU seeds).
 //   The kernel accumulates sum S q with q = exp(+i theta), theta = 2 pi frac(phi);
 //   exp(-2 pi i phi) = conj(q), so the epilogue stores (re, -im).
 //
@@ -62,15 +65,17 @@ namespace {
 #define WALK_CTAS 4
 #endif
 constexpr int WTHREADS = WALK_THREADS;   // (baseline, time) pairs per CTA
-constexpr int WH = WALK_FT / 2;      // chain length
-constexpr int WJ0 = WH / 2 - 1;      // seed position (and WJ0 + 1)
+constexpr int WH = WALK_FT / 2;      // steps each way = packed accumulator pairs per thread
+constexpr int WJ0 = WH - 1;          // seed position (and WJ0 + 1): the middle of the 32-channel chain
+// step t of the walk: lane 0 is at channel WJ0 + 1 + t (forward), lane 1 at channel WJ0 - t (backward)
+__host__ __device__ constexpr int walk_chan(int t, int lane) { return lane ? WJ0 - t : WJ0 + 1 + t; }
 
 // one launch's constants: per component its geometry record and 16 flux words (S[j], S[j + WH]),
 // interleaved so that every constant-bank offset in the loop body is a small immediate
 template <typename Geo>
 struct WalkRec {
     Geo geo;
-    ulonglong2 flux[WH / 2];          // 128-bit granule q = words 2q, 2q + 1
+    ulonglong2 flux[WH / 2];          // 128-bit granule q = words 2q, 2q + 1; word t = (S[J0+1+t], S[J0-t])
 };
 template <typename Geo>
 struct WalkBlock {
@@ -90,39 +95,42 @@ struct WParams {
     int k0, n_k;                     // first record of this launch's block in the bank; components in it
     int load_acc;                    // 1: continue from the values in vis, 0: start from zero
     int first;                       // first block of the call: range violations are counted once
-    double sfA, sfB, ds, smax;       // nu/c at the two seed channels, channel step / c, max |nu/c| of the tile
+    double sf0, ds, smax;            // nu/c at the seed channel J0, channel step / c, max |nu/c| of the tile
     unsigned int *err;               // device-side precondition counter (woden_check)
 };
 
-// sign pattern of the recurrence: s_j = +1 for (j - J0) mod 4 in {0, 1}, else -1
-__host__ __device__ constexpr bool walk_neg(int j) { return (((j - WJ0) % 4 + 4) % 4) >= 2; }
+// sign pattern of the recurrence: s_j = +1 for (j - J0) mod 4 in {0, 1}, else -1; at step t both lanes
+// (j - J0 = 1 + t and -t) carry the same sign
+__host__ __device__ constexpr bool walk_neg(int t) { return (t & 3) == 1 || (t & 3) == 2; }
+static_assert(!walk_neg(0) && walk_neg(1) && walk_neg(2) && !walk_neg(3), "sign pattern");
 
 template <bool GAUSS>
 struct Seed {
-    float cA, sA, cB, sB;     // q at position J0 of chain A (lane 0) and chain B (lane 1)
-    float wr, wi;             // exp(i delta)
+    float r0, i0, r1, i1;     // q at positions J0 and J0 + 1
+    float wr;                 // cos(delta)
     float Q;                  // Gaussian: metres-domain quadratic form
 };
 
 template <bool GAUSS, typename Geo>
 __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, double w, float uf, float vf,
-                                          double sfA, double ds, double magic, int kshift, float qmax, Seed<GAUSS> &sd)
+                                          double sf0, double ds, double magic, int kshift, float qmax, Seed<GAUSS> &sd)
 {
     // S3: D = u l + v m + w (n-1), FP64 metres
     const double D = fma(u, g.l, fma(v, g.m, w * g.n1));
     // frac(phase) as signed Q0.32: the low word of phase + 1.5*2^(20+k) holds the phase modulo 2^k
     // turns in units of 2^(k-32) turn, so a left shift by k leaves the fraction (k = 0 while the
-    // thread's phases stay below 2^19 turns; see phase_shift_for).  Chain A's seed and the channel
-    // step by one DFMA each; chain B's seed, WH channels up, by integer arithmetic (wraps mod 1 turn)
-    const unsigned qA = (unsigned)__double2loint(fma(D, sfA, magic)) << kshift;
+    // thread's phases stay below 2^19 turns; see phase_shift_for).  The seed and the channel step by
+    // one DFMA each.
+    const unsigned q0 = (unsigned)__double2loint(fma(D, sf0, magic)) << kshift;
     const unsigned qd = (unsigned)__double2loint(fma(D, ds, magic)) << kshift;
-    const unsigned qB = qA + (unsigned)WH * qd;
-    const float thA = (float)(int)qA * Q32_TO_RAD;
-    const float thB = (float)(int)qB * Q32_TO_RAD;
+    const float th0 = (float)(int)q0 * Q32_TO_RAD;
     const float thd = (float)(int)qd * Q32_TO_RAD;
-    sd.cA = __cosf(thA); sd.sA = __sinf(thA);
-    sd.cB = __cosf(thB); sd.sB = __sinf(thB);
-    sd.wr = __cosf(thd); sd.wi = __sinf(thd);
+    sd.r0 = __cosf(th0); sd.i0 = __sinf(th0);
+    const float wi = __sinf(thd);
+    sd.wr = __cosf(thd);
+    // position J0 + 1 by one complex rotation with w = exp(i delta)
+    sd.r1 = fmaf(-sd.i0, wi, sd.r0 * sd.wr);
+    sd.i1 = fmaf(sd.r0, wi, sd.i0 * sd.wr);
     if constexpr (GAUSS) {
         // Eq 13-14 in metres: gx = cg maj (sin pa u + cos pa v), gy = cg min (cos pa u - sin pa v)
         const float gx = fmaf(g.as, uf, g.ac * vf);
@@ -135,13 +143,15 @@ __device__ __forceinline__ void make_seed(const Geo &g, double u, double v, doub
 
 // Gaussian envelope constants of a thread (per chain lane): exponents in units of Q
 struct EnvConst {
-    f32x2 e0, ef, eb;   // xi at J0; forward ratio J0 -> J0+1; backward ratio J0 -> J0-1
-    float e2;           // second difference
-    // Largest Q this thread walks with: Q |ef|, Q |eb| <= 126, so every step ratio 2^(Q e) is finite.
-    // Where the clamp bites, xi at J0 is 2^(-126 |e0| / |eb|) with |e0| / |eb| ~ s / (2 ds) >= 32 (the
-    // walking path is only taken when a chain spans at most +-12.5 % in frequency, api.cu): it has
-    // flushed to zero, as has the true envelope at every channel of the chain (< 2^-90), and the chain
-    // is an exact 0 instead of 0 x inf = NaN.  Otherwise the clamp is idle.
+    f32x2 e0, er;       // lanes (forward, backward): xi at (J0+1, J0); first ratio (J0+1 -> J0+2, J0 -> J0-1)
+    float e2;           // second difference (the same in both directions)
+    // Largest Q this thread walks with: Q |er| <= 126 in both lanes, so the first step ratios 2^(Q e) are
+    // finite; the ratio that is > 1 (towards lower |nu|) only shrinks along the walk, the other one only
+    // underflows.  Where the clamp bites, xi at the seeds is 2^(-126 |e0| / |er|) with |e0| / |er| ~
+    // s / (2 ds) >= 32 (the walking path is only taken when the channel step is at most 1/64 of the lowest
+    // frequency, api.cu): it has flushed to zero, as has the true envelope at every channel of the chain
+    // (at its far end |nu| is still >= 0.75 of the seed's: < 2^-2000), and the chain is an exact 0 instead
+    // of 0 x inf = NaN.  Otherwise the clamp is idle.
     float qmax;
 };
 
@@ -149,7 +159,7 @@ template <bool GAUSS>
 __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const WParams p)
 {
     using Geo = typename std::conditional<GAUSS, GeoG, GeoP>::type;
-    constexpr int FT = WALK_FT, H = WH, J0 = WJ0;
+    constexpr int FT = WALK_FT, H = WH;
     // the bank as one array of records; k0 is a run-time value on purpose: the record index then
     // carries the half's base and every constant-bank offset below is a small immediate
     const WalkRec<Geo> *const rec = reinterpret_cast<const WalkRec<Geo> *>(CBANK);
@@ -162,7 +172,7 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     double u = 0.0, v = 0.0, w = 0.0;
     if (valid) { u = p.u_m[bt]; v = p.v_m[bt]; w = p.w_m[bt]; }
     const float uf = (float)u, vf = (float)v;
-    const double sfA = p.sfA, sfB = p.sfB, ds = p.ds;
+    const double sf0 = p.sf0, ds = p.ds;
     // phase range of this thread: |D nu/c| <= sqrt(2) |b| max(nu)/c turns (l^2 + m^2 < 1)
     int kshift = phase_shift_for(sqrt(fma(u, u, fma(v, v, w * w))) * 1.4142135623730951 * p.smax);
     if (kshift > PHASE_MAX_SHIFT) {              // beyond 2^28 turns: counted for woden_check
@@ -172,16 +182,15 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     const double magic = magic32_shifted(kshift);
 
     EnvConst ec;
-    ec.e0 = ec.ef = ec.eb = 0ull; ec.e2 = 0.f; ec.qmax = 0.f;
+    ec.e0 = ec.er = 0ull; ec.e2 = 0.f; ec.qmax = 0.f;
     if constexpr (GAUSS) {
         // exponent(s) = -Q s^2, s_j = s_J0 + (j - J0) ds
-        const float e0A = (float)(-sfA * sfA), e0B = (float)(-sfB * sfB);
-        const float efA = (float)(-(2.0 * sfA * ds + ds * ds)), efB = (float)(-(2.0 * sfB * ds + ds * ds));
-        const float ebA = (float)(2.0 * sfA * ds - ds * ds), ebB = (float)(2.0 * sfB * ds - ds * ds);
-        ec.e0 = pack2(e0A, e0B); ec.ef = pack2(efA, efB); ec.eb = pack2(ebA, ebB);
+        const double s1 = sf0 + ds;
+        const float e0f = (float)(-s1 * s1), e0b = (float)(-sf0 * sf0);
+        const float erf = (float)(-(2.0 * s1 * ds + ds * ds)), erb = (float)(2.0 * sf0 * ds - ds * ds);
+        ec.e0 = pack2(e0f, e0b); ec.er = pack2(erf, erb);
         ec.e2 = (float)(-2.0 * ds * ds);
-        const float emax = fmaxf(fmaxf(fabsf(efA), fabsf(efB)), fmaxf(fabsf(ebA), fabsf(ebB)));
-        ec.qmax = fminf(126.f / emax, 1.0e30f);
+        ec.qmax = fminf(126.f / fmaxf(fabsf(erf), fabsf(erb)), 1.0e30f);
     }
 
     // accumulators: y_j = s_j x_j of q = conj(exp(-2 pi i phi)); the output holds V = (s re, -s im),
@@ -193,9 +202,10 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     if (p.load_acc) {
 #pragma unroll
         for (int j = 0; j < H; ++j) {
+            const int jf = walk_chan(j, 0), jb = walk_chan(j, 1);
             float2 a = make_float2(0.f, 0.f), c = make_float2(0.f, 0.f);
-            if (valid && p.ftile * FT + j < p.F) a = row[(size_t)j * p.B];
-            if (valid && p.ftile * FT + j + H < p.F) c = row[(size_t)(j + H) * p.B];
+            if (valid && p.ftile * FT + jf < p.F) a = row[(size_t)jf * p.B];
+            if (valid && p.ftile * FT + jb < p.F) c = row[(size_t)jb * p.B];
             const float sg = walk_neg(j) ? -1.f : 1.f;
             acc_re[j] = pack2(sg * a.x, sg * c.x);
             acc_im[j] = pack2(-sg * a.y, -sg * c.y);
@@ -206,72 +216,56 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
     }
 
     Seed<GAUSS> sd;
-    make_seed<GAUSS>(rec[k0].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, ec.qmax, sd);
-#pragma unroll 2
+    make_seed<GAUSS>(rec[k0].geo, u, v, w, uf, vf, sf0, ds, magic, kshift, ec.qmax, sd);
+    constexpr int UNROLL_K = GAUSS ? 4 : 2;      // measured: points 205.6 ms at 2 (206.9 at 4), Gaussians 89.4 at 4 (91.0 at 2)
+#pragma unroll UNROLL_K
     for (int k = k0; k < k1; ++k) {
         // software pipeline: the seed (FP64 + MUFU) of component k+1 overlaps the FP32 walk of k
         Seed<GAUSS> nx;
-        make_seed<GAUSS>(rec[k + 1 < k1 ? k + 1 : k].geo, u, v, w, uf, vf, sfA, ds, magic, kshift, ec.qmax, nx);
+        make_seed<GAUSS>(rec[k + 1 < k1 ? k + 1 : k].geo, u, v, w, uf, vf, sf0, ds, magic, kshift, ec.qmax, nx);
 
-        // word j = (S[j], S[j + H]), read as 128-bit granules into uniform registers
+        // word t = (S[J0+1+t], S[J0-t]), read as 128-bit granules into uniform registers
         const ulonglong2 *fl = rec[k].flux;
         const float cf = sd.wr + sd.wr;                    // c = 2 cos(delta)
         const f32x2 c2 = pack2(cf, cf), nc2 = pack2(-cf, -cf);
-        const f32x2 wr = pack2(sd.wr, sd.wr), wi = pack2(sd.wi, sd.wi), nwi = pack2(-sd.wi, -sd.wi);
-        // positions J0 (MUFU) and J0 + 1 (one complex rotation); s_J0 = s_{J0+1} = +1
-        const f32x2 r0 = pack2(sd.cA, sd.cB), i0 = pack2(sd.sA, sd.sB);
-        const f32x2 r1 = fma2(i0, nwi, mul2(r0, wr));
-        const f32x2 i1 = fma2(r0, wi, mul2(i0, wr));
 
-        f32x2 xf = 0ull, rf = 0ull, xb = 0ull, rb = 0ull, qq = 0ull;
+        f32x2 x = 0ull, r = 0ull, qq = 0ull;
         if constexpr (GAUSS) {
             float a, b2;
             const f32x2 Q2 = pack2(sd.Q, sd.Q);
             unpack2(mul2(Q2, ec.e0), a, b2);
-            xb = pack2(ex2_approx(a), ex2_approx(b2));                // xi at J0
-            // step ratios: finite because Q <= ec.qmax (see EnvConst)
-            unpack2(mul2(Q2, ec.ef), a, b2);
-            rf = pack2(ex2_approx(a), ex2_approx(b2));                // xi_{J0+1} / xi_{J0}
-            unpack2(mul2(Q2, ec.eb), a, b2);
-            rb = pack2(ex2_approx(a), ex2_approx(b2));                // xi_{J0-1} / xi_{J0}
+            x = pack2(ex2_approx(a), ex2_approx(b2));                 // xi at (J0+1, J0)
+            // first step ratios: finite because Q <= ec.qmax (see EnvConst)
+            unpack2(mul2(Q2, ec.er), a, b2);
+            r = pack2(ex2_approx(a), ex2_approx(b2));                 // xi_{J0+2} / xi_{J0+1}, xi_{J0-1} / xi_{J0}
             const float qf = ex2_approx(sd.Q * ec.e2);
             qq = pack2(qf, qf);
-            xf = mul2(xb, rf);                                        // xi at J0 + 1
-            rf = mul2(rf, qq);                                        // ratio J0+1 -> J0+2
         }
 
-        // ---- both directions in lock step: forward y_{j+1} = (s_{j+1} s_j) c y_j + y_{j-1} over positions
-        // J0+1 .. H-1, backward y_{j-1} = (s_{j-1} s_j) c y_j + y_{j+1} over J0 .. 0.  At step t the
-        // forward chain sits at jf = J0 + 1 + t and the backward chain at jb = J0 - t; the sign pattern is
-        // symmetric about J0 + 1/2, so the four recurrence FMAs of a step share one scalar (+c or -c).
+        // ---- both directions in the two lanes: y_{t+1} = (s_{t+1} s_t) c y_t + y_{t-1}, forward over channels
+        // J0+1 .. 31 in lane 0 and backward over J0 .. 0 in lane 1; at t = 0 the "previous" value of each
+        // lane is the other lane's seed.
         {
-            f32x2 fra = r0, fia = i0, frc = r1, fic = i1;      // forward: previous, current
-            f32x2 bra = r1, bia = i1, brc = r0, bic = i0;      // backward
+            f32x2 ra = pack2(sd.r0, sd.r1), rc = pack2(sd.r1, sd.r0);      // previous, current
+            f32x2 ia = pack2(sd.i0, sd.i1), ic = pack2(sd.i1, sd.i0);
 #pragma unroll
-            for (int t = 0; t < H / 2; ++t) {
-                const int jf = J0 + 1 + t, jb = J0 - t;
-                static_assert(H == 2 * (J0 + 1), "chains are walked symmetrically");
-                f32x2 frn = 0ull, fin = 0ull, brn = 0ull, bin = 0ull;
-                const bool more = t + 1 < H / 2;
-                const bool flip = walk_neg(jf + 1) != walk_neg(jf);
-                const f32x2 cc = flip ? nc2 : c2;           // same for jb - 1 vs jb (symmetry)
-                f32x2 Sf = (jf & 1) ? fl[jf >> 1].y : fl[jf >> 1].x;
-                f32x2 Sb = (jb & 1) ? fl[jb >> 1].y : fl[jb >> 1].x;
+            for (int t = 0; t < H; ++t) {
+                f32x2 rn = 0ull, in = 0ull;
+                const bool more = t + 1 < H;
+                const bool flip = walk_neg(t + 1) != walk_neg(t);
+                const f32x2 cc = flip ? nc2 : c2;
+                f32x2 S = (t & 1) ? fl[t >> 1].y : fl[t >> 1].x;
                 if constexpr (GAUSS) {
-                    Sf = mul2(Sf, xf); Sb = mul2(Sb, xb);
-                    if (more) { xf = mul2(xf, rf); rf = mul2(rf, qq); xb = mul2(xb, rb); rb = mul2(rb, qq); }
+                    S = mul2(S, x);
+                    if (more) { x = mul2(x, r); r = mul2(r, qq); }
                 }
-                // each recurrence is followed by the accumulate of the same chain value (shared operand)
-                if (more) frn = fma2(frc, cc, fra);
-                acc_re[jf] = fma2(frc, Sf, acc_re[jf]);
-                if (more) fin = fma2(fic, cc, fia);
-                acc_im[jf] = fma2(fic, Sf, acc_im[jf]);
-                if (more) brn = fma2(brc, cc, bra);
-                acc_re[jb] = fma2(brc, Sb, acc_re[jb]);
-                if (more) bin = fma2(bic, cc, bia);
-                acc_im[jb] = fma2(bic, Sb, acc_im[jb]);
-                fra = frc; fia = fic; frc = frn; fic = fin;
-                bra = brc; bia = bic; brc = brn; bic = bin;
+                // source order measured best (profiles/walk_rf_r3.md): ptxas keeps each chain's recurrence and
+                // accumulate adjacent (shared slot-A operand) and pairs slightly better from this order
+                if (more) rn = fma2(rc, cc, ra);
+                if (more) in = fma2(ic, cc, ia);
+                acc_im[t] = fma2(ic, S, acc_im[t]);
+                acc_re[t] = fma2(rc, S, acc_re[t]);
+                ra = rc; ia = ic; rc = rn; ic = in;
             }
         }
         sd = nx;
@@ -285,8 +279,9 @@ __global__ void __launch_bounds__(WTHREADS, WALK_CTAS) predict_walk_kernel(const
             unpack2(acc_re[j], a0, a1);
             unpack2(acc_im[j], b0, b1);
             const float sg = walk_neg(j) ? -1.f : 1.f;
-            if (p.ftile * FT + j < p.F) row[(size_t)j * p.B] = make_float2(sg * a0, -sg * b0);
-            if (p.ftile * FT + j + H < p.F) row[(size_t)(j + H) * p.B] = make_float2(sg * a1, -sg * b1);
+            const int jf = walk_chan(j, 0), jb = walk_chan(j, 1);
+            if (p.ftile * FT + jf < p.F) row[(size_t)jf * p.B] = make_float2(sg * a0, -sg * b0);
+            if (p.ftile * FT + jb < p.F) row[(size_t)jb * p.B] = make_float2(sg * a1, -sg * b1);
         }
     }
 }
@@ -305,7 +300,7 @@ __global__ void pack_walk_blocks_kernel(const Geo *__restrict__ geo, const doubl
     const int pos = (int)(i % WALK_FT);
     const long long r = i / WALK_FT;
     const int k = (int)(r % n), ftile = (int)(r / n);
-    const int j = (pos >> 1) + (pos & 1) * WH;               // lane 0: channel pos/2, lane 1: + WH
+    const int j = walk_chan(pos >> 1, pos & 1);              // word t = pos / 2: lane 0 forward, lane 1 backward
     const int f = ftile * WALK_FT + j;
     WalkBlock<Geo> *blk = reinterpret_cast<WalkBlock<Geo> *>(blocks + ((size_t)ftile * n_chunks + k / KC) * WALK_CB_BYTES);
     float val = 0.f;
@@ -376,8 +371,7 @@ cudaError_t launch(const UvwDev &uvw, const ChanTable &ch, const unsigned char *
         p.bt1 = n_ftiles >= 2 ? n_bt : (unit == 0 ? (half_bt < n_bt ? half_bt : n_bt) : n_bt);
         if (p.bt1 <= p.bt0) continue;
         p.ftile = ftile;
-        p.sfA = ch.s_host[ftile * WALK_FT + WJ0];
-        p.sfB = ch.s_host[ftile * WALK_FT + WH + WJ0];
+        p.sf0 = ch.s_host[ftile * WALK_FT + WJ0];
         const double sa = ch.s_host[ftile * WALK_FT], sb = ch.s_host[ftile * WALK_FT + WALK_FT - 1];
         p.smax = sa > sb ? sa : sb;
         const unsigned grid = (unsigned)((p.bt1 - p.bt0 + WTHREADS - 1) / WTHREADS);

@@ -74,3 +74,17 @@ def test_per_type_labels_follow_the_order_step_runs_the_predictors():
     assert rec["labels_consistent"]
     wrong = dict(ms, points=18.5, gaussians=641.0, shapelets=241.0)
     assert not bench.general_path_record(wrong, counts, mufu, 0.85, 1, sum(counts.values()), 5)["labels_consistent"]
+
+
+def test_read_cycle_model_rule_on_a_hand_written_sass_excerpt():
+    # the register-file read-cycle figures quoted in profiles/ come from a committed
+    # command (`bench.py --rf-model`); its counting rule is pinned here line by line
+    sys.path.insert(0, ROOT)
+    import bench
+    text = open(os.path.join(ROOT, "tests", "golden", "sass_read_cycle_excerpt.txt")).read()
+    m = bench.read_cycle_model(text, "toy_kernel")
+    assert m["instructions"] == 9 and m["packed_fp32"] == 4
+    assert m["per_opcode"]["FFMA2"] == 3 + 1 + 2 + 3
+    assert m["per_opcode"]["DFMA"] == 2 and m["per_opcode"]["MUFU.COS"] == 1
+    assert m["per_opcode"].get("LDCU.64", 0) == 0
+    assert m["read_cycles"] == 12
