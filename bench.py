@@ -39,11 +39,11 @@ MUFU_LANES_PER_SM = 16          # measured: profiles/pipes_r1.md
 FP32_LANES_PER_SM = 128
 SM_MAX_HZ = 1965e6
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on config 5, recorded
-# from the ncu --set full captures summarised in profiles/ncu_r2_kernels.md (not measured in this run):
+# from the ncu --set full captures summarised in profiles/ncu_r3_kernels.md (not measured in this run):
 # (component type, path) -> (kernel, bytes, commit the capture was taken at)
 NCU_DRAM_BYTES = {
-    ("points", "walk"): ("predict_walk_kernel<false>", 10981376 + 70713088, "4acabf5"),
-    ("gaussians", "walk"): ("predict_walk_kernel<true>", 10989312 + 76573952, "4acabf5"),
+    ("points", "walk"): ("predict_walk_kernel<false>", 11120384 + 66082048, "13aa7d5"),
+    ("gaussians", "walk"): ("predict_walk_kernel<true>", 10993408 + 70302464, "13aa7d5"),
 }
 KERNEL_NAMES = {("points", "walk"): "predict_walk_kernel<false>", ("gaussians", "walk"): "predict_walk_kernel<true>",
                 ("points", "general"): "predict_pg_kernel<16, false>", ("gaussians", "general"): "predict_pg_kernel<16, true>",
@@ -415,7 +415,7 @@ def run_ours(args):
     basis, peak = ops["walk" if walk else "general"]
     ach = (per_type[dominant]["coeff_evals_per_s"] if dominant == "shapelets"
            else per_type[dominant]["evals_per_s"])
-    # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r2_kernels.md):
+    # DRAM bytes of the dominant kernel per launch (ncu --set full, profiles/ncu_r3_kernels.md):
     # the visibility buffer once, plus the component blocks that miss L2
     key = (dominant, "walk" if walk else "general")
     rec_traffic = NCU_DRAM_BYTES.get(key) if args.config == 5 else None
@@ -426,7 +426,7 @@ def run_ours(args):
         "unit": "Gevals/s", "frac": ach / peak,
         "traffic": rec_traffic[1] if rec_traffic else None,
         "traffic_source": (f"ncu --set full capture of one launch of {rec_traffic[0]} at commit {rec_traffic[2]} "
-                           "(profiles/ncu_r2_kernels.md): a recorded constant, not measured in this run")
+                           "(profiles/ncu_r3_kernels.md): a recorded constant, not measured in this run")
         if rec_traffic else None,
         "achieved_basis": "evals of the whole woden_predict_* call / its CUDA-event duration (the call is a sequence "
                           "of launches of this kernel plus three O(K) staging kernels)",

@@ -303,7 +303,10 @@ int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, doub
  * weights: DEVICE [n] (the integrated flux density of a point source or Gaussian; Eq 25's weight of a
  * shapelet basis function).  keep: DEVICE int [n], 1 for a kept component, else 0; n_keep: DEVICE
  * int [1] = N_comp.  f_comp >= 1 keeps everything; the running sum is formed in ranked order in FP64 and
- * compared with f_comp * total * (1 + 1e-15).  0 <= n <= 2^20 (ranking is by counting, O(n^2)). */
+ * compared with f_comp * total * (1 + 1e-15).  0 <= n <= 2^17 (ranking is by counting, O(n^2): 0.1 s at the
+ * limit; the paper's models have 7656 components).  A non-finite weight ranks as 0 (last) and is
+ * counted for woden_check() (WODEN_ERR_DATA); woden_truncate_select_static ranks it the same way but has no
+ * context to report it through. */
 int woden_truncate_select(woden_ctx *ctx, int n, const double *weights, double f_comp, int *keep, int *n_keep,
                           void *cuda_stream);
 

@@ -848,17 +848,20 @@ int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, doub
 int woden_truncate_select(woden_ctx *ctx, int n, const double *weights, double f_comp, int *keep, int *n_keep, void *cuda_stream)
 {
     if (!ctx) return WODEN_ERR_NULL;
-    if (n < 0 || n > (1 << 20) || !(f_comp >= 0.0)) return WODEN_ERR_DIM;
+    if (n < 0 || n > (1 << 17) || !(f_comp >= 0.0)) return WODEN_ERR_DIM;
     if (!n_keep || (n > 0 && (!weights || !keep))) return WODEN_ERR_NULL;
     Bind bind(ctx);
     if (!bind.ok) return WODEN_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     ctx->last_stream = st;
     if (n == 0) { CU(ctx, cudaMemsetAsync(n_keep, 0, sizeof(int), st), "truncate zero"); return WODEN_OK; }
+    int rc = ensure_err(ctx, st);
+    if (rc != WODEN_OK) return rc;
     CU(ctx, ctx->f_small.reserve((size_t)n * 12 + 64), "alloc truncation scratch");
     double *sorted = static_cast<double *>(ctx->f_small.p);
     int *rank = reinterpret_cast<int *>(sorted + n);
-    CU(ctx, launch_truncate_select(weights, n, f_comp, rank, sorted, keep, n_keep, st), "truncate launch");
+    CU(ctx, launch_truncate_select(weights, n, f_comp, rank, sorted, keep, n_keep,
+                                   static_cast<unsigned int *>(ctx->err.p), st), "truncate launch");
     return WODEN_OK;
 }
 

@@ -127,7 +127,7 @@ cudaError_t launch_fit_basis_sums(const FitProblem &f, const FitScratch &w, doub
 
 // ---- model truncation (truncate.cu, Eq 23-24) ---------------------
 cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
-                                   int *n_keep, cudaStream_t st);
+                                   int *n_keep, unsigned int *err, cudaStream_t st);
 
 // ---- pipe microbenchmarks (pipes.cu) -----------------------------------------------------
 cudaError_t run_pipe_rate(int which, int iters, double *thread_ops_per_s, double *sm_clock_hz);

@@ -11,14 +11,20 @@
 namespace woden {
 namespace {
 
-__global__ void trunc_rank_kernel(const double *__restrict__ w, int n, int *__restrict__ rank, double *__restrict__ sorted)
+// |I_j| as ranked: a non-finite weight (NaN would make the order partial and leave slots of the ranked list
+// unwritten) counts as 0 -- it ranks last -- and is reported through the context's error counter
+__device__ __forceinline__ double trunc_abs(double w) { return isfinite(w) ? fabs(w) : 0.0; }
+
+__global__ void trunc_rank_kernel(const double *__restrict__ w, int n, int *__restrict__ rank, double *__restrict__ sorted,
+                                  unsigned int *__restrict__ err)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
-    const double a = fabs(w[j]);
+    if (!isfinite(w[j])) atomicAdd(err, 1u);
+    const double a = trunc_abs(w[j]);
     int r = 0;
     for (int i = 0; i < n; ++i) {
-        const double b = fabs(w[i]);
+        const double b = trunc_abs(w[i]);
         r += (b > a) || (b == a && i < j);
     }
     rank[j] = r;
@@ -50,9 +56,9 @@ __global__ void trunc_flag_kernel(const int *__restrict__ rank, int n, const int
 }  // namespace
 
 cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
-                                   int *n_keep, cudaStream_t st)
+                                   int *n_keep, unsigned int *err, cudaStream_t st)
 {
-    trunc_rank_kernel<<<(n + 127) / 128, 128, 0, st>>>(weights, n, rank, sorted); note_launch();
+    trunc_rank_kernel<<<(n + 127) / 128, 128, 0, st>>>(weights, n, rank, sorted, err); note_launch();
     trunc_count_kernel<<<1, 32, 0, st>>>(sorted, n, f_comp, n_keep); note_launch();
     trunc_flag_kernel<<<(n + 255) / 256, 256, 0, st>>>(rank, n, n_keep, keep); note_launch();
     return cudaGetLastError();

@@ -66,15 +66,18 @@ int scratch_for_current_device(StaticScratch **out)
     return WODEN_OK;
 }
 
+// as in truncate.cu: a non-finite weight ranks as 0 (there is no context here whose counter could report it)
+__device__ __forceinline__ double static_abs(double w) { return isfinite(w) ? fabs(w) : 0.0; }
+
 // rank_j = number of components with a larger |I| (equal values in their original order): Eq 24
 __global__ void static_rank_kernel(const double *__restrict__ w, int n, StaticScratch *__restrict__ s)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
-    const double a = fabs(w[j]);
+    const double a = static_abs(w[j]);
     int r = 0;
     for (int i = 0; i < n; ++i) {
-        const double b = fabs(w[i]);
+        const double b = static_abs(w[i]);
         r += (b > a) || (b == a && i < j);
     }
     s->rank[j] = r;
@@ -127,8 +130,8 @@ int woden_truncate_select_static(int n, const double *weights, double f_comp, in
     StaticScratch *s = nullptr;
     int rc = scratch_for_current_device(&s);
     if (rc != WODEN_OK) return rc;
-    // the array still holds the previous call's ranked list: start this call's part of it from zero so
-    // that no slot the ranking leaves unwritten (possible only with NaN weights) carries old values
+    // the array still holds the previous call's ranked list: start this call's part of it from zero, so that
+    // whatever the weights are, nothing of an earlier call can enter this call's running sum
     e = cudaMemsetAsync(s->sorted, 0, sizeof(double) * (size_t)n, st);
     if (e != cudaSuccess) return fail(WODEN_ERR_CUDA, "clear static scratch", e);
     static_rank_kernel<<<(n + 127) / 128, 128, 0, st>>>(weights, n, s); woden::note_launch();

@@ -480,3 +480,24 @@ def test_p16_uv_basis_is_rephasing_to_the_component_centre():
             assert np.allclose(got[0], uj[0], atol=1e-9) and np.allclose(got[1], vj[0], atol=1e-9)
     # the generator's matrices (used for configs 1, 4, 5) are the same ones
     assert np.allclose(inputs.local_uv_basis(l, m, d0), oracle.shapelet_uv_basis(l, m, d0), atol=1e-15)
+
+
+def test_oracle_uv_basis_equals_the_generators_independent_construction():
+    # predict_workload and the CUDA side each compute M_j (reading G4) with their own routine
+    # from (l, m, dec0); the generator builds it a third way (cross products with the celestial pole in numpy,
+    # inputs.local_uv_basis).  Pin the oracle's routine to the generator's arrays for the shapelet configs, so a
+    # misreading of the basis rotation shared by the two C-side routines cannot pass end-to-end parity unnoticed.
+    for cfg in (4, 5, 6):
+        wl = inputs.make_config(cfg)
+        s = wl.shapelets
+        assert s.n > 0 and s.uv_basis is not None
+        M = oracle.shapelet_uv_basis(s.l, s.m, wl.meta["dec0_rad"])
+        assert M.shape == s.uv_basis.reshape(s.n, 6).shape
+        assert np.max(np.abs(M - s.uv_basis.reshape(s.n, 6))) <= 1e-12
+        # and it is not the identity-like trivial case: the rows are orthonormal 3-vectors orthogonal to s
+        for j in range(s.n):
+            e, nvec = M[j, :3], M[j, 3:]
+            n_dir = np.sqrt(1.0 - s.l[j] ** 2 - s.m[j] ** 2)
+            sdir = np.array([s.l[j], s.m[j], n_dir])
+            assert abs(e @ e - 1) < 1e-12 and abs(nvec @ nvec - 1) < 1e-12 and abs(e @ nvec) < 1e-12
+            assert abs(e @ sdir) < 1e-12 and abs(nvec @ sdir) < 1e-12

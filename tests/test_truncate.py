@@ -85,6 +85,34 @@ def test_gpu_selection_is_bit_exact_against_the_oracle(ctx):
 
 
 @pytest.mark.gpu
+def test_gpu_selection_with_non_finite_weights_is_defined_and_reported(ctx):
+    # a NaN weight would make the ranking a partial order (slots of the ranked list never written); the library
+    # ranks non-finite weights as 0, counts them for woden_check, and the rest of the list is selected as usual
+    import torch
+    from paper_2005_09316_b200 import binding
+    rng = np.random.default_rng(10)
+    w = rng.normal(0, 1, 300) * rng.lognormal(0, 1, 300)
+    bad = w.copy()
+    bad[[3, 77, 150]] = np.nan
+    bad[[5, 200]] = [np.inf, -np.inf]
+    as_zero = np.where(np.isfinite(bad), bad, 0.0)
+    ctx.check()
+    for f in (0.2, 0.7, 1.0):
+        keep, nk = ctx.truncate_select(torch.as_tensor(bad, device="cuda:0"), f)
+        ref = otrunc.keep_mask(as_zero, f)
+        assert np.array_equal(keep.cpu().numpy().astype(bool), ref)
+        assert int(nk[0]) == int(ref.sum())
+        with pytest.raises(binding.WodenError) as e:
+            ctx.check()
+        assert e.value.status == binding.WODEN_ERR_DATA
+        k2 = torch.empty(300, dtype=torch.int32, device="cuda:0"); n2 = torch.empty(1, dtype=torch.int32, device="cuda:0")
+        binding.truncate_select_static(torch.as_tensor(bad, device="cuda:0"), f, k2, n2)
+        assert torch.equal(k2, keep) and int(n2[0]) == int(nk[0])
+    keep, nk = ctx.truncate_select(torch.as_tensor(w, device="cuda:0"), 0.5)     # finite input: nothing reported
+    ctx.check()
+
+
+@pytest.mark.gpu
 def test_gpu_eq25_basis_sums_match_the_oracle(ctx):
     # sum_pixels |(G * B_q)| for every basis function: with and without the beam, rotated, rectangular pixels
     for p_max, beam in ((6, None), (9, (1.5 * ARCMIN, 1.0 * ARCMIN, 0.7, 6)), (20, (1.0 * ARCMIN, 1.0 * ARCMIN, 0.0, 4))):
