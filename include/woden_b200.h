@@ -296,6 +296,26 @@ int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, doub
                               int p_max, double beta1_rad, double beta2_rad, const woden_restoring_beam *beam,
                               double *abs_sums, void *cuda_stream);
 
+/* Eq 25 for a whole shapelet model that was NOT fitted by woden_fit_shapelets (which returns
+ * these weights itself): weights[i] = |coeff[i] s0_jy[j]| x sum over pixels of |(G * B_{n1[i], n2[i]})| for every
+ * listed basis function i of every component j, the sums being woden_shapelet_basis_sums of component j (order =
+ * the highest n1 + n2 in its list, its beta1 / beta2 / pa) on the grid and beam below.  The paper sums over "the
+ * pixels used during the model fit" with the restoring beam G; a model whose coefficients were not fitted to an
+ * image has neither, so a grid and a beam are part of the call (reading G20): n_pix x n_pix pixels centred
+ * on the component, spanning +-1.5 sqrt(2 p + 1) max(beta1, beta2) / (2 sqrt(2 ln 2)) per axis (1.5 x the highest
+ * order's turning point), and a circular Gaussian beam of FWHM beam_fwhm_rad sampled to +-min(24, ceil(1.5 FWHM /
+ * pixel)) pixels.  n_pix <= 0 selects WODEN_EQ25_PIXELS, beam_fwhm_rad < 0 selects WODEN_EQ25_BEAM_FWHM_RAD (about
+ * the resolution of a 3 km array at 180 MHz), beam_fwhm_rad == 0 means no beam.
+ * s0_jy, beta1_rad, beta2_rad, pa_rad: HOST [n]; coeff_offset: HOST [n + 1] (CSR, coeff_offset[0] = 0); n1, n2,
+ * coeff: HOST [coeff_offset[n]]; weights: DEVICE [coeff_offset[n]] (ready for woden_truncate_select).  Orders above
+ * WODEN_MAX_ORDER: WODEN_ERR_ORDER; 3 <= n_pix <= 2048. */
+#define WODEN_EQ25_PIXELS        257
+#define WODEN_EQ25_BEAM_FWHM_RAD (2.0 * 3.14159265358979323846 / 10800.0)   /* 2 arcmin */
+int woden_shapelet_truncation_weights(woden_ctx *ctx, int n, const double *s0_jy, const double *beta1_rad,
+                                      const double *beta2_rad, const double *pa_rad, const int *coeff_offset,
+                                      const int *n1, const int *n2, const double *coeff, int n_pix,
+                                      double beam_fwhm_rad, double *weights, void *cuda_stream);
+
 /* Model truncation, section 5.3 (Eq 23-24, :273-275): with the n
  * components ranked by |weights[j]|, largest first (equal values in their original order), keep the
  * largest N_comp whose summed absolute weight does not exceed f_comp times the total,

@@ -26,6 +26,7 @@ WODEN_ERR_DATA = -6
 WODEN_ERR_STATIC_LIMIT = -7
 WODEN_MAX_ORDER = 100
 WODEN_STATIC_TRUNCATE_MAX = 16384
+WODEN_EQ25_PIXELS = 257
 WODEN_PATH_AUTO = 0
 WODEN_PATH_GENERAL = 1
 WODEN_PATH_NONE = -1
@@ -44,7 +45,7 @@ EXPORTS = ["woden_create", "woden_destroy", "woden_strerror", "woden_last_error"
            "woden_set_path", "woden_last_path", "woden_last_shapelet_path", "woden_last_shapelet_bucket", "woden_kernel_launches", "woden_predict_points", "woden_predict_gaussians",
            "woden_predict_shapelets", "woden_simulate_host", "woden_pipe_rate",
            "woden_uvw_from_antennas", "woden_shapelet_uv_basis", "woden_calibrate_gains", "woden_peel", "woden_set_shapelet_path", "woden_shapelet_series", "woden_fit_shapelets", "woden_fit_gram_ms", "woden_shapelet_basis_sums",
-           "woden_truncate_select", "woden_truncate_select_static", "woden_static_last_error"]
+           "woden_shapelet_truncation_weights", "woden_truncate_select", "woden_truncate_select_static", "woden_static_last_error"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
@@ -125,6 +126,8 @@ def load() -> C.CDLL:
     L.woden_shapelet_basis_sums.argtypes = [_vp, C.POINTER(woden_image_grid), C.c_double, C.c_double, C.c_double, C.c_int,
                                             C.c_double, C.c_double, C.POINTER(woden_restoring_beam), _vp, _vp]
     L.woden_truncate_select.argtypes = [_vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp]
+    L.woden_shapelet_truncation_weights.argtypes = [_vp, C.c_int, _dp, _dp, _dp, _dp, _ip, _ip, _ip, _dp, C.c_int,
+                                                    C.c_double, _vp, _vp]
     L.woden_truncate_select_static.argtypes = [C.c_int, _vp, C.c_double, _vp, _vp, _vp]
     L.woden_static_last_error.restype = C.c_char_p
     L.woden_static_last_error.argtypes = []
@@ -399,6 +402,25 @@ class Woden:
                                                float(beta1_rad), float(beta2_rad), C.byref(cb) if cb is not None else None,
                                                _ptr(out), _stream_handle(stream))
         self._ck(rc, "woden_shapelet_basis_sums")
+        return out
+
+    def shapelet_truncation_weights(self, s0_jy, beta1_rad, beta2_rad, pa_rad, coeff_offset, n1, n2, coeff,
+                                    n_pix: int = 0, beam_fwhm_rad: float = -1.0, stream=None):
+        """woden_shapelet_truncation_weights (Eq 25) on HOST arrays: device float64 [n_coeff] of weights.
+        n_pix = 0 / beam_fwhm_rad < 0 take the header's defaults (reading G20)."""
+        import torch
+        a = [_hd(x) for x in (s0_jy, beta1_rad, beta2_rad, pa_rad)]
+        off, i1, i2 = (np.ascontiguousarray(x, dtype=np.int32) for x in (coeff_offset, n1, n2))
+        cf = _hd(coeff)
+        n = int(a[0].size)
+        if off.size != n + 1 or i1.size != cf.size or i2.size != cf.size or (n and int(off[-1]) != cf.size):
+            raise ValueError("inconsistent CSR coefficient lists")
+        out = torch.empty(int(cf.size), dtype=torch.float64, device=f"cuda:{self.device}")
+        ip = lambda x: None if x.size == 0 else x.ctypes.data_as(_ip)
+        rc = self._L.woden_shapelet_truncation_weights(self._ctx, n, *[_hdp(x) for x in a], ip(off), ip(i1), ip(i2),
+                                                       _hdp(cf), int(n_pix), float(beam_fwhm_rad),
+                                                       _ptr(out) if cf.size else None, _stream_handle(stream))
+        self._ck(rc, "woden_shapelet_truncation_weights")
         return out
 
     def truncate_select(self, weights, f_comp: float, stream=None):

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libwoden_b200.so (include/woden_b200.h): argument validation, the
 // context's grow-only device scratch, the per-call channel table, and kernel sequencing.
 // Host code only; every step of the hot path runs in the kernels it launches.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -43,6 +44,7 @@ struct woden_ctx {
     std::string last_error;
     DevBuf geo, flux, tri, chan, err, hang, bmat, bscale, lut, wblocks;
     DevBuf f_hx, f_a0, f_at, f_small, f_gram, f_ops, f_part;     // woden_fit_shapelets scratch
+    DevBuf t_list, t_sums;                                       // woden_shapelet_truncation_weights staging
     int lut_pm = -1, lut_nx = 0;
     double lut_dx = 0.0;
     int shapelet_path = WODEN_SHAPELET_AUTO;
@@ -842,6 +844,72 @@ int woden_shapelet_basis_sums(woden_ctx *ctx, const woden_image_grid *grid, doub
     if (rc != WODEN_OK) return rc;
     f.beta1 = beta1_rad; f.beta2 = beta2_rad;
     CU(ctx, launch_fit_basis_sums(f, w, abs_sums, st), "basis sums launch");
+    return WODEN_OK;
+}
+
+int woden_shapelet_truncation_weights(woden_ctx *ctx, int n, const double *s0_jy, const double *beta1_rad,
+                                      const double *beta2_rad, const double *pa_rad, const int *coeff_offset,
+                                      const int *n1, const int *n2, const double *coeff, int n_pix,
+                                      double beam_fwhm_rad, double *weights, void *cuda_stream)
+{
+    if (!ctx) return WODEN_ERR_NULL;
+    if (n < 0) return WODEN_ERR_DIM;
+    if (n == 0) return WODEN_OK;
+    if (!s0_jy || !beta1_rad || !beta2_rad || !pa_rad || !coeff_offset) return WODEN_ERR_NULL;
+    const int n_coeff = coeff_offset[n];
+    if (coeff_offset[0] != 0 || n_coeff < 0) return WODEN_ERR_DIM;
+    for (int j = 0; j < n; ++j)
+        if (coeff_offset[j + 1] < coeff_offset[j]) return WODEN_ERR_DIM;
+    if (n_coeff == 0) return WODEN_OK;
+    if (!n1 || !n2 || !coeff || !weights) return WODEN_ERR_NULL;
+    if (n_pix <= 0) n_pix = WODEN_EQ25_PIXELS;
+    if (beam_fwhm_rad < 0.0) beam_fwhm_rad = WODEN_EQ25_BEAM_FWHM_RAD;
+    if (n_pix < 3 || n_pix > 2048 || !std::isfinite(beam_fwhm_rad)) return WODEN_ERR_DIM;
+    Bind bind(ctx);
+    if (!bind.ok) return WODEN_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    ctx->last_stream = st;
+    int rc = ensure_err(ctx, st);
+    if (rc != WODEN_OK) return rc;
+    // the coefficient lists go to the device once (pageable source: staged by the runtime before the call returns)
+    const size_t ints = ((size_t)n_coeff * sizeof(int) + 7) / 8 * 8;
+    CU(ctx, ctx->t_list.reserve(2 * ints + (size_t)n_coeff * sizeof(double)), "alloc coefficient lists");
+    unsigned char *base = static_cast<unsigned char *>(ctx->t_list.p);
+    int *d_n1 = reinterpret_cast<int *>(base), *d_n2 = reinterpret_cast<int *>(base + ints);
+    double *d_cf = reinterpret_cast<double *>(base + 2 * ints);
+    CU(ctx, cudaMemcpyAsync(d_n1, n1, (size_t)n_coeff * sizeof(int), cudaMemcpyHostToDevice, st), "upload n1");
+    CU(ctx, cudaMemcpyAsync(d_n2, n2, (size_t)n_coeff * sizeof(int), cudaMemcpyHostToDevice, st), "upload n2");
+    CU(ctx, cudaMemcpyAsync(d_cf, coeff, (size_t)n_coeff * sizeof(double), cudaMemcpyHostToDevice, st), "upload coefficients");
+    const double a = 2.0 * std::sqrt(2.0 * std::log(2.0));
+    for (int j = 0; j < n; ++j) {
+        const int lo = coeff_offset[j], hi = coeff_offset[j + 1];
+        if (hi == lo) continue;
+        int pm = 0;
+        for (int i = lo; i < hi; ++i) {
+            if (n1[i] < 0 || n2[i] < 0 || n1[i] + n2[i] > WODEN_MAX_ORDER) return WODEN_ERR_ORDER;
+            pm = std::max(pm, n1[i] + n2[i]);
+        }
+        if (!(beta1_rad[j] > 0.0) || !(beta2_rad[j] > 0.0) || !std::isfinite(beta1_rad[j]) || !std::isfinite(beta2_rad[j]))
+            return WODEN_ERR_DIM;
+        // reading G20: n_pix^2 pixels over +-1.5 sqrt(2 pm + 1) max(beta) / a per axis, centred on the component
+        const double half = 1.5 * std::sqrt(2.0 * pm + 1.0) * std::max(beta1_rad[j], beta2_rad[j]) / a;
+        const double pix = 2.0 * half / (n_pix - 1);
+        woden_image_grid grid{n_pix, n_pix, -pix, pix, 0.0, 0.0};
+        woden_restoring_beam beam{beam_fwhm_rad, beam_fwhm_rad, 0.0, 0};
+        if (beam_fwhm_rad > 0.0) beam.half_width = (int)std::min(24.0, std::ceil(1.5 * beam_fwhm_rad / pix));
+        FitScratch w;
+        FitProblem f;
+        FitSizes sz;
+        rc = fit_setup(ctx, &grid, 0.0, 0.0, pa_rad[j], pm, beam_fwhm_rad > 0.0 ? &beam : nullptr, false, st, &w, &f, &sz);
+        if (rc != WODEN_OK) return rc;
+        f.beta1 = beta1_rad[j]; f.beta2 = beta2_rad[j];
+        const int P = (pm + 1) * (pm + 2) / 2;
+        CU(ctx, ctx->t_sums.reserve((size_t)P * sizeof(double)), "alloc basis sums");
+        double *sums = static_cast<double *>(ctx->t_sums.p);
+        CU(ctx, launch_fit_basis_sums(f, w, sums, st), "basis sums launch");
+        CU(ctx, launch_eq25_weights(d_cf + lo, d_n1 + lo, d_n2 + lo, hi - lo, pm, s0_jy[j], sums, weights + lo,
+                                    static_cast<unsigned int *>(ctx->err.p), st), "Eq 25 weights launch");
+    }
     return WODEN_OK;
 }
 

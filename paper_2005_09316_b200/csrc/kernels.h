@@ -126,6 +126,8 @@ cudaError_t launch_fit_argmin(const double *residual, int n, int *best, cudaStre
 cudaError_t launch_fit_basis_sums(const FitProblem &f, const FitScratch &w, double *abs_sums, cudaStream_t st);
 
 // ---- model truncation (truncate.cu, Eq 23-24) ---------------------
+cudaError_t launch_eq25_weights(const double *coeff, const int *n1, const int *n2, int count, int pm, double s0,
+                                const double *abs_sums, double *weights, unsigned int *err, cudaStream_t st);
 cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
                                    int *n_keep, unsigned int *err, cudaStream_t st);
 

@@ -53,7 +53,30 @@ __global__ void trunc_flag_kernel(const int *__restrict__ rank, int n, const int
     if (j < n) keep[j] = rank[j] < *n_keep ? 1 : 0;
 }
 
+// Eq 25 for the listed basis functions of ONE shapelet component: weight_i = |C_i S0| x the
+// beam-convolved basis image's absolute pixel sum of (n1_i, n2_i) (abs_sums over the full triangle of order pm,
+// n1-major: q = n1 (pm + 1) - n1 (n1 - 1) / 2 + n2).  An order pair outside the triangle gets weight 0 and is counted.
+__global__ void eq25_weight_kernel(const double *__restrict__ coeff, const int *__restrict__ n1, const int *__restrict__ n2,
+                                   int count, int pm, double s0, const double *__restrict__ abs_sums,
+                                   double *__restrict__ weights, unsigned int *__restrict__ err)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const int a = n1[i], b = n2[i];
+    if (a < 0 || b < 0 || a + b > pm) { weights[i] = 0.0; atomicAdd(err, 1u); return; }
+    const int q = a * (pm + 1) - a * (a - 1) / 2 + b;
+    weights[i] = fabs(coeff[i] * s0) * abs_sums[q];
+}
+
 }  // namespace
+
+cudaError_t launch_eq25_weights(const double *coeff, const int *n1, const int *n2, int count, int pm, double s0,
+                                const double *abs_sums, double *weights, unsigned int *err, cudaStream_t st)
+{
+    if (count <= 0) return cudaSuccess;
+    eq25_weight_kernel<<<(count + 255) / 256, 256, 0, st>>>(coeff, n1, n2, count, pm, s0, abs_sums, weights, err); note_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_truncate_select(const double *weights, int n, double f_comp, int *rank, double *sorted, int *keep,
                                    int *n_keep, unsigned int *err, cudaStream_t st)

@@ -128,6 +128,59 @@ def test_gpu_eq25_basis_sums_match_the_oracle(ctx):
 
 
 @pytest.mark.gpu
+def test_gpu_eq25_weights_of_a_whole_model_match_the_oracle(ctx):
+    # woden_shapelet_truncation_weights: |C S0| x sum_pixels |G * B| per listed basis function on the grid and beam
+    # of reading G20, against the image-space oracle on the same grid; ragged, unsorted lists,
+    # an empty component, no beam / default beam / explicit beam
+    from paper_2005_09316_b200 import binding
+    rng = np.random.default_rng(21)
+    a = 2.0 * np.sqrt(2.0 * np.log(2.0))
+    s0 = np.array([1.5, -0.7, 2.0]); b1 = np.array([3.0, 5.0, 2.0]) * ARCMIN; b2 = np.array([2.0, 6.5, 2.0]) * ARCMIN
+    pa = np.array([0.4, 2.1, 0.0])
+    lists = [[(0, 0), (3, 2), (1, 7), (9, 0), (2, 2)], [], [(0, 12), (5, 5), (0, 0), (11, 1)]]
+    off = np.cumsum([0] + [len(x) for x in lists]).astype(np.int32)
+    n1 = np.array([p[0] for x in lists for p in x], dtype=np.int32)
+    n2 = np.array([p[1] for x in lists for p in x], dtype=np.int32)
+    cf = rng.normal(0, 1, n1.size)
+    for n_pix, fwhm in ((65, 0.0), (65, 1.5 * ARCMIN)):
+        got = ctx.shapelet_truncation_weights(s0, b1, b2, pa, off, n1, n2, cf, n_pix=n_pix, beam_fwhm_rad=fwhm)
+        got = got.cpu().numpy()
+        npx, beam_fwhm = n_pix, fwhm
+        ref = np.zeros(cf.size)
+        for j in range(3):
+            lo, hi = off[j], off[j + 1]
+            if hi == lo:
+                continue
+            pm = int((n1[lo:hi] + n2[lo:hi]).max())
+            half = 1.5 * np.sqrt(2 * pm + 1.0) * max(b1[j], b2[j]) / a
+            pix = 2.0 * half / (npx - 1)
+            kw = {}
+            if beam_fwhm > 0:
+                kw = dict(bmaj=beam_fwhm, bmin=beam_fwhm, bpa=0.0, half_width=int(min(24, np.ceil(1.5 * beam_fwhm / pix))))
+            A = shamfi.design_matrix(npx, npx, -pix, pix, 0.0, 0.0, 0.0, 0.0, pa[j], b1[j], b2[j], pm, **kw)
+            full = np.zeros(A.shape[1])
+            q = n1[lo:hi].astype(np.int64) * (pm + 1) - n1[lo:hi].astype(np.int64) * (n1[lo:hi] - 1) // 2 + n2[lo:hi]
+            for i, qi in zip(range(lo, hi), q):
+                full[:] = 0.0
+                full[qi] = cf[i] * s0[j]
+                ref[i] = shamfi.truncation_weights(full, A)[qi]
+        assert np.abs(got - ref).max() <= 1e-10 * ref.max(), (n_pix, fwhm)
+    ctx.check()
+    # the defaults of reading G20 are what the header says: 257 pixels, a 2 arcmin beam
+    dflt = ctx.shapelet_truncation_weights(s0, b1, b2, pa, off, n1, n2, cf)
+    expl = ctx.shapelet_truncation_weights(s0, b1, b2, pa, off, n1, n2, cf, n_pix=binding.WODEN_EQ25_PIXELS,
+                                           beam_fwhm_rad=2.0 * ARCMIN)
+    import torch
+    assert torch.equal(dflt, expl) and float(dflt.min()) > 0.0
+    empty = ctx.shapelet_truncation_weights(s0[:0], b1[:0], b2[:0], pa[:0], np.zeros(1, np.int32), n1[:0], n2[:0], cf[:0])
+    assert empty.numel() == 0
+    with pytest.raises(binding.WodenError) as e:
+        ctx.shapelet_truncation_weights(s0[:1], b1[:1], b2[:1], pa[:1], np.array([0, 1], np.int32), np.array([60], np.int32),
+                                        np.array([60], np.int32), np.array([1.0]))
+    assert e.value.status == binding.WODEN_ERR_ORDER
+
+
+@pytest.mark.gpu
 def test_components_and_shapelets_are_truncated_consistently(ctx):
     from paper_2005_09316_b200 import truncate
     wl = inputs.make_config(4)               # MS-CLEAN-like: 25 % negative components
@@ -139,10 +192,11 @@ def test_components_and_shapelets_are_truncated_consistently(ctx):
     full = truncate.truncate_components(ctx, wl.points, 1.0)
     assert full.n == wl.points.n and np.array_equal(full.l, wl.points.l)
     s = inputs.make_config(5).shapelets
-    w = truncate.shapelet_basis_weights(ctx, s)
+    w_dev = truncate.shapelet_basis_weights(ctx, s)          # Eq 25 by the library; stays on the device
+    w = w_dev.cpu().numpy()
     assert w.shape == s.coeff.shape and (w >= 0).all() and w.max() > 0
     for f in (1.0, 0.6, 0.2):
-        t = truncate.truncate_shapelets(ctx, s, f, w)
+        t = truncate.truncate_shapelets(ctx, s, f, w_dev)
         assert t.coeff_offset[0] == 0 and t.coeff_offset[-1] == t.coeff.size == t.n1.size == t.n2.size
         assert np.all(np.diff(t.coeff_offset) >= 0) and t.n == s.n
         if f == 1.0:
